@@ -1,0 +1,217 @@
+"""Pins of the oracle's whole step: invariants, closed forms, analytic dam breaks."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle.swe_oracle import OracleSolver
+from paper_2010_14416_b200 import workloads as W
+from tests.analytic import ritter_profile, stoker, stoker_profile
+
+G = 9.81
+
+
+def _l1(hnum, hexact, area):
+    return float(np.sum(np.abs(hnum - hexact) * area) / np.sum(area))
+
+
+# ------------------------------------------------------------------ well-balancedness
+def test_lake_at_rest_variable_bed_with_islands():
+    """R-13/R-14: rest over 64 bumps, some emergent, is kept to round-off (config 3 shape)."""
+    w = W.config3(nx=120, ny=60, nsteps=300)
+    s = OracleSolver.from_workload(w)
+    geo = s.geometry()
+    dry0 = w.h <= w.h_dry
+    assert 0.005 < dry0.mean() < 0.6, "the reduced config must keep emergent islands"
+    dt0 = s.compute_dt()
+    s.run(300)
+    h, hu, hv, _, dt = s.get_state()
+    wet = h > w.h_dry
+    np.testing.assert_array_equal(~wet, dry0)
+    u = np.where(wet, hu / np.where(wet, h, 1.0), 0.0)
+    v = np.where(wet, hv / np.where(wet, h, 1.0), 0.0)
+    assert np.abs(u).max() < 1e-10 and np.abs(v).max() < 1e-10
+    assert np.abs(h[wet] + geo["z"][wet] - 2.0).max() < 1e-12
+    assert dt == pytest.approx(dt0, rel=1e-12)
+    assert s.stats()["nclamp"] == 0
+
+
+def test_wrong_source_factor_would_not_be_at_rest():
+    """The lake-at-rest pin is sharp: the step's momentum residual comes from cancelling the
+    edge pressure g h**^2/2 against eq.(30) with g/2; here we check the two pieces separately
+    are O(1), so a lost factor (R-13) or sign could not pass the test above."""
+    w = W.config3(nx=40, ny=20)
+    flat = W.config3(nx=40, ny=20)
+    flat.bathymetry = np.zeros_like(flat.bathymetry)      # same depths, flat bed: not at rest
+    s = OracleSolver.from_workload(flat)
+    s.run(1)
+    _, hu, hv, _, _ = s.get_state()
+    assert max(np.abs(hu).max(), np.abs(hv).max()) > 1e-3
+    s = OracleSolver.from_workload(w)
+    s.run(1)
+    _, hu, hv, _, _ = s.get_state()
+    assert max(np.abs(hu).max(), np.abs(hv).max()) < 1e-13
+
+
+def test_flat_bed_rest_to_roundoff():
+    """Equal depths on a flat bed: every edge returns exactly (0, g h^2/2, 0) (R-12), so the
+    only residual is the closure sum_k L_k n_k = 0 in floating point (a few ulp per step)."""
+    w = W.canal_dam_break(30, 5, h_left=0.8, h_right=0.8, manning=0.03, length=30.0)
+    s = OracleSolver.from_workload(w)
+    s.run(50)
+    h, hu, hv, _, _ = s.get_state()
+    assert np.abs(h - 0.8).max() < 1e-14
+    assert max(np.abs(hu).max(), np.abs(hv).max()) < 1e-14
+
+
+# ------------------------------------------------------------------ conservation
+@pytest.mark.parametrize("hr,mn", [(0.5, 0.0), (0.0, 0.03)])
+def test_mass_conservation_closed_box(hr, mn):
+    w = W.canal_dam_break(100, 10, h_left=1.0, h_right=hr, manning=mn, seed=20102)
+    s = OracleSolver.from_workload(w)
+    v0 = s.stats()["volume"]
+    s.run(500)
+    st = s.stats()
+    assert st["nclamp"] == 0
+    assert st["volume"] == pytest.approx(v0, rel=1e-12)
+    assert st["boundary_volume_out"] == 0.0
+
+
+def test_inflow_outflow_mass_balance():
+    """R-20: d/dt sum h|Omega| = Q_in - outflow, to round-off (river-shaped small domain)."""
+    w = W.config4(nx=120, ny=30, nsteps=300)
+    s = OracleSolver.from_workload(w)
+    v0 = s.stats()["volume"]
+    s.run(300)
+    st = s.stats()
+    h, hu, hv, t, _ = s.get_state()
+    assert st["nclamp"] == 0 and t > 0
+    assert st["volume"] - v0 == pytest.approx(-st["boundary_volume_out"], rel=1e-9, abs=1e-9 * v0)
+    # nothing has reached the outlet yet, so the gain is exactly the prescribed discharge
+    right_wet = (W.centroids(w.nodes_xy, w.tris)[:, 0] > 0.98 * w.nodes_xy[:, 0].max()) & (hu > 1e-9)
+    if not right_wet.any():
+        assert st["volume"] - v0 == pytest.approx(500.0 * t, rel=1e-9)
+
+
+# ------------------------------------------------------------------ friction
+def test_friction_closed_form_uniform_flow():
+    """eq.(33)-(37): uniform h and q, flat bed, transmissive box: one step gives exactly
+    q' = q / (1 + dt c |q|), c = g m^2 h^(-7/3), direction preserved (SURVEY 8(c) pin)."""
+    w = W.canal_dam_break(12, 6, h_left=0.9, h_right=0.9, manning=0.035, length=12.0)
+    w.bc_tags[w.bc_tags > 0] = W.BC_TRANSMISSIVE
+    q = np.array([0.6, -0.35])
+    w.hu[:] = q[0]
+    w.hv[:] = q[1]
+    s = OracleSolver.from_workload(w)
+    dt = 0.37
+    s.step_dt(dt)
+    h, hu, hv, _, _ = s.get_state()
+    c = G * 0.035 ** 2 * 0.9 ** (-7.0 / 3.0)
+    f = 1.0 / (1.0 + dt * c * np.linalg.norm(q))
+    np.testing.assert_allclose(h, 0.9, rtol=1e-13)
+    np.testing.assert_allclose(hu, q[0] * f, rtol=1e-12)
+    np.testing.assert_allclose(hv, q[1] * f, rtol=1e-12)
+
+
+def test_zero_manning_is_the_explicit_scheme():
+    w0 = W.canal_dam_break(40, 6, manning=0.0, length=40.0, seed=3)
+    w1 = W.canal_dam_break(40, 6, manning=1e-30, length=40.0, seed=3)
+    a, b = OracleSolver.from_workload(w0), OracleSolver.from_workload(w1)
+    a.run(40)
+    b.run(40)
+    for x, y in zip(a.get_state()[:3], b.get_state()[:3]):
+        np.testing.assert_allclose(x, y, rtol=1e-13, atol=1e-15)
+
+
+def test_friction_decelerates_and_h_column_sign():
+    """With friction the dam-break front is slower; momentum magnitude never grows by friction."""
+    w0 = W.canal_dam_break(100, 4, h_right=0.0, manning=0.0, seed=5)
+    w1 = W.canal_dam_break(100, 4, h_right=0.0, manning=0.05, seed=5)
+    a, b = OracleSolver.from_workload(w0), OracleSolver.from_workload(w1)
+    a.run(200)
+    b.run(200)
+    cx = W.centroids(w0.nodes_xy, w0.tris)[:, 0]
+    fa = cx[a.get_state()[0] > 1e-3].max()
+    fb = cx[b.get_state()[0] > 1e-3].max()
+    assert fb < fa
+
+
+# ------------------------------------------------------------------ time step
+def test_dt_closed_form_uniform_state():
+    """eq.(15), R-9: dt = CFL R_min / (sqrt(g h) + |V|) on a uniform state."""
+    w = W.canal_dam_break(20, 5, h_left=1.7, h_right=1.7, length=20.0)
+    w.hu[:] = 1.7 * 0.8
+    w.hv[:] = -1.7 * 0.6
+    s = OracleSolver.from_workload(w)
+    rmin = s.geometry()["rin"].min()
+    assert s.compute_dt() == pytest.approx(0.9 * rmin / (math.sqrt(G * 1.7) + 1.0), rel=1e-14)
+    # inradius: R = 2 |Omega| / perimeter
+    geo = s.geometry()
+    np.testing.assert_allclose(geo["rin"], 2 * geo["area"] / geo["len"].sum(1), rtol=1e-15)
+
+
+def test_all_dry_gives_zero_dt_and_no_steps():
+    w = W.canal_dam_break(10, 3, h_left=0.0, h_right=0.0, length=10.0)
+    s = OracleSolver.from_workload(w)
+    assert s.compute_dt() == 0.0
+    assert s.run(5) == 0
+
+
+# ------------------------------------------------------------------ analytic dam breaks
+def _run_until(s, t_end, chunk=10):
+    while s.get_state()[3] < t_end:
+        s.run(chunk)
+    return s.get_state()
+
+
+@pytest.mark.parametrize("hL,hR,t_end", [(1.0, 0.5, 8.0), (10.0, 1.0, 2.5)])
+def test_stoker_convergence(hL, hR, t_end):
+    """Wet-wet dam break against the Stoker solution (BASELINE config 1; paper's 10 | 1 case,
+    PAPER.md:485-491): L1(h) error decreases with dx at the first-order-scheme rate, plateau
+    depth within 1 %."""
+    errs = []
+    for nx in (100, 200, 400):
+        w = W.canal_dam_break(nx, 4, h_left=hL, h_right=hR, seed=20102)
+        s = OracleSolver.from_workload(w)
+        h, hu, hv, t, _ = _run_until(s, t_end)
+        cx = W.centroids(w.nodes_xy, w.tris)[:, 0]
+        hex_, _ = stoker_profile((cx - 50.0) / t, hL, hR)
+        errs.append(_l1(h, hex_, s.geometry()["area"]))
+        if nx == 400:
+            p = stoker(hL, hR)
+            xi = (cx - 50.0) / t
+            plateau = (xi > p["tail"] + 0.25 * (p["shock"] - p["tail"])) & \
+                      (xi < p["shock"] - 0.25 * (p["shock"] - p["tail"]))
+            assert np.abs(h[plateau] / p["hm"] - 1.0).max() < 0.01
+            u = hu[plateau] / h[plateau]
+            assert np.abs(u / p["um"] - 1.0).max() < 0.02
+            assert s.stats()["nclamp"] == 0
+    assert errs[1] < 0.72 * errs[0] and errs[2] < 0.72 * errs[1]
+    assert errs[2] < 0.012 * hL
+
+
+def test_ritter_front_and_profile():
+    """Frictionless wet-dry dam break (config 2 variant, m = 0) against Ritter."""
+    errs, tips = [], []
+    for nx in (200, 400):
+        w = W.canal_dam_break(nx, 4, h_left=1.0, h_right=0.0, manning=0.0, seed=20103)
+        s = OracleSolver.from_workload(w)
+        h, hu, hv, t, _ = _run_until(s, 5.0)
+        cx = W.centroids(w.nodes_xy, w.tris)[:, 0]
+        hex_, _ = ritter_profile((cx - 50.0) / t, 1.0)
+        errs.append(_l1(h, hex_, s.geometry()["area"]))
+        # front position: the h = 5 cm contour within 3 %; the thin tip (1 cm contour) is known
+        # to lag in first-order schemes and must approach the exact position under refinement
+        ratios = []
+        for thr in (5e-2, 1e-2):
+            front = cx[h > thr].max() - 50.0
+            exact = t * (2.0 * math.sqrt(G) - 3.0 * math.sqrt(G * thr))
+            ratios.append(front / exact)
+        assert ratios[0] == pytest.approx(1.0, abs=0.03)
+        assert 0.85 < ratios[1] < 1.0
+        tips.append(ratios[1])
+        assert s.stats()["nclamp"] == 0
+        # upstream of the rarefaction head only numerical diffusion has arrived
+        assert np.abs(h[cx < 50.0 - 1.05 * math.sqrt(G) * t - 2.0] - 1.0).max() < 0.01
+    assert errs[1] < 0.75 * errs[0]
+    assert tips[1] > tips[0]
