@@ -1,0 +1,185 @@
+/*
+ * swe.h -- C ABI of libswe_b200: the time-explicit cell-centred finite-volume step of the
+ * 2-D Shallow-Water Equations on an unstructured triangular mesh, FP64, one B200 (sm_100a).
+ *
+ * Method: Delmas & Soulaimani, arXiv 2010.14416, sections 2-3:
+ *   state U = (h, hu, hv) per triangle (eq.1), explicit Euler finite volumes
+ *   (eq.6-16), HLLC flux per edge in the rotated frame (PAPER.md:111-123
+ *   eq.12-14, :141-189 eq.17-26), bathymetry by hydrostatic reconstruction (PAPER.md:196-217
+ *   eq.28-30), semi-implicit Manning friction (eq.31-37), boundary fluxes
+ *   (PAPER.md:125), CFL time step with the inscribed-circle radius (eq.15)
+ *   reduced on the device.  Readings of garbled passages: DESIGN.md section 4.
+ *
+ * Conventions
+ *   - Every function returns SWE_OK (0) or a negative swe_status; nothing throws across the
+ *     ABI.  swe_last_error(mesh) gives a message for the last failure on that handle
+ *     (swe_last_error(NULL): last failure of swe_mesh_create in this thread).
+ *   - "host" pointers are ordinary CPU memory, caller-owned, read or written during the call
+ *     only.  "device" pointers are CUDA device memory of the bound device, caller-owned.
+ *   - Cells are addressed in the CALLER's numbering everywhere in this ABI; the internal
+ *     locality renumbering (swe_params.ordering) is invisible except via swe_get_permutation.
+ *   - Local edge k (0,1,2) of a triangle joins its vertices k and (k+1) mod 3.
+ *   - A handle is not thread-safe.  All device work is issued on the stream given to
+ *     swe_mesh_bind_device; swe_step / swe_run are asynchronous on that stream.
+ *   - There is no CPU fallback: every compute entry point fails with SWE_ERR_NOT_BOUND or
+ *     SWE_ERR_CUDA when no device workspace is bound or CUDA is unavailable.
+ */
+#ifndef SWE_B200_H
+#define SWE_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct swe_mesh swe_mesh; /* opaque */
+
+typedef enum {
+    SWE_OK = 0,
+    SWE_ERR_INVALID_ARG = -1,   /* NULL pointer, non-positive size, bad enum value */
+    SWE_ERR_BAD_INDEX = -2,     /* triangle refers to a node outside [0, nn) */
+    SWE_ERR_DEGENERATE = -3,    /* zero-area triangle */
+    SWE_ERR_NON_MANIFOLD = -4,  /* an edge is shared by more than two triangles */
+    SWE_ERR_BAD_VALUE = -5,     /* NaN/inf coordinate, bed or state; negative Manning or depth */
+    SWE_ERR_NOT_BOUND = -6,     /* no device workspace bound yet */
+    SWE_ERR_WORKSPACE = -7,     /* workspace too small or misaligned */
+    SWE_ERR_CUDA = -8,          /* a CUDA call failed (message in swe_last_error) */
+    SWE_ERR_ALL_DRY = -9,       /* every cell is dry: no time step can be defined */
+    SWE_ERR_NO_STATE = -10,     /* swe_set_state has not been called */
+    SWE_ERR_BAD_TAG = -11,      /* boundary tag out of range or without edges */
+    SWE_ERR_NOMEM = -12
+} swe_status;
+
+/* boundary tags of bc_tags */
+enum { SWE_BC_WALL = 1, SWE_BC_TRANSMISSIVE = 2, SWE_BC_INFLOW0 = 3, SWE_BC_MAX_TAG = 127 };
+/* swe_params.ordering: create-time renumbering of the cells for gather locality */
+enum { SWE_ORDER_IDENTITY = 0, SWE_ORDER_HILBERT = 1, SWE_ORDER_RCM = 2 };
+/* swe_params.loop_mode: how swe_run iterates without host round trips */
+enum { SWE_LOOP_AUTO = 0, SWE_LOOP_GRAPH = 1, SWE_LOOP_PERSISTENT = 2, SWE_LOOP_LAUNCH = 3 };
+
+typedef struct {
+    double g;           /* gravitational acceleration; the paper gives no value, default 9.81 */
+    double cfl;         /* CFL number of eq.(15); default 0.9 */
+    double h_dry;       /* wet/dry threshold: a cell or edge side is dry iff h <= h_dry; 1e-6 */
+    int32_t ordering;   /* SWE_ORDER_*; default SWE_ORDER_HILBERT */
+    int32_t block_size; /* CUDA threads per block, multiple of 32 in [64, 1024]; 0 = default */
+    int32_t loop_mode;  /* SWE_LOOP_*; default SWE_LOOP_AUTO */
+    int32_t reserved;   /* must be 0 */
+} swe_params;
+
+typedef struct {
+    double volume;        /* sum_i h_i |Omega_i| (m^3), summed on the host in long double */
+    double t;             /* simulated time */
+    double dt_last;       /* time step used by the most recent step (0 before the first) */
+    int64_t steps;        /* steps taken since swe_set_state */
+    int64_t n_dry;        /* cells with h <= h_dry */
+    int64_t n_clamped;    /* times a negative depth was clamped to 0 (R-15; expected 0) */
+    int64_t n_nonfinite;  /* cells whose state is NaN/inf (expected 0) */
+} swe_stats;
+
+/* Fills *p with the defaults listed above. */
+int swe_params_default(swe_params *p);
+
+/*
+ * Builds the mesh tables on the host (Fig. 4 gives the input format: node
+ * table x, y, z and connectivity table of three node ids + Manning coefficient per cell).
+ *   nodes_xy    host [nn][2]  node coordinates (m)
+ *   tris        host [nt][3]  node ids per triangle; clockwise triangles are re-oriented by
+ *                             swapping vertices 1 and 2 (their edge tags follow)
+ *   bathymetry  host [nn]     bed elevation z per node; the cell bed is the mean of its three
+ *                             node values (R-1)
+ *   manning     host [nt]     Manning coefficient m per cell, >= 0 (eq.5)
+ *   bc_tags     host [nt][3]  boundary tag per local edge, read only where the edge has no
+ *                             neighbour; <= 0 or missing means SWE_BC_WALL
+ *   params      host          NULL = defaults
+ * Tables built (SoA, in the internal cell order): neighbour index per edge, unit outward
+ * normal, L_ij / |Omega_i|, 1 / R_i, g m^2, cell bed.  nt < 2^31.  No CUDA call is made.
+ */
+int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_t nt,
+                    const double *bathymetry, const double *manning, const int8_t *bc_tags,
+                    const swe_params *params, swe_mesh **out);
+
+/* Frees the host tables and CUDA graphs.  Never frees the caller's device workspace. */
+int swe_mesh_destroy(swe_mesh *mesh);
+
+/* Bytes of device memory the mesh needs (tables + two state buffers + staging). */
+int swe_mesh_workspace_bytes(const swe_mesh *mesh, size_t *bytes);
+
+/*
+ * Binds caller-provided device memory (>= workspace bytes, 256-byte aligned, on the current
+ * CUDA device) and a CUDA stream (cudaStream_t as void*, NULL = default stream), uploads the
+ * tables.  The memory must stay valid until swe_mesh_destroy or a new bind.
+ */
+int swe_mesh_bind_device(swe_mesh *mesh, void *device_workspace, size_t bytes, void *cuda_stream);
+
+/*
+ * Prescribed inflow (R-20): total discharge Q (m^3/s, positive into the domain)
+ * over all boundary edges carrying `tag` (>= SWE_BC_INFLOW0); each edge gets the unit
+ * discharge -Q / sum(L) along its outward normal.  Call after swe_mesh_create, any time.
+ */
+int swe_set_bc_value(swe_mesh *mesh, int tag, double total_discharge);
+
+/*
+ * Sets U = (h, hu, hv) and the time.  host / device [nt] each, caller numbering.  Requires
+ * h >= 0 and finite values (checked on the host variant).  Momentum of dry cells (h <= h_dry)
+ * is discarded (R-15).  Resets the step counter; the time step becomes stale.
+ */
+int swe_set_state(swe_mesh *mesh, const double *h, const double *hu, const double *hv, double t0);
+int swe_set_state_device(swe_mesh *mesh, const double *d_h, const double *d_hu, const double *d_hv,
+                         double t0);
+
+/*
+ * Time step of the CURRENT state, eq.(15) with d = R_i, reduced on the device
+ * (PAPER.md:457): dt = CFL / max_i (sqrt(g h_i) + |V_i|) / R_i over wet cells.  Synchronises the
+ * stream.  Leaves dt on the device for the next step.  SWE_ERR_ALL_DRY if no cell is wet.
+ */
+int swe_compute_dt(swe_mesh *mesh, double *dt_out);
+
+/* One step (eq.37) with the device-resident dt, then the next dt. = swe_run(mesh, 1) */
+int swe_step(swe_mesh *mesh);
+
+/*
+ * nsteps steps, asynchronous, no host<->device traffic inside: each step gathers the three
+ * neighbours, computes the three edge fluxes with sources and friction, writes U^{n+1} to the
+ * other state buffer and the per-block maximum of (sqrt(g h)+|V|)/R for the next dt.
+ * If the domain becomes all dry the remaining steps leave the state unchanged (dt = 0).
+ */
+int swe_run(swe_mesh *mesh, int64_t nsteps);
+
+/* Waits for the stream. */
+int swe_sync(swe_mesh *mesh);
+
+/*
+ * Reads the state back in caller numbering.  Any of h, hu, hv, t, dt_next may be NULL.
+ * dt_next is the step the next swe_step would use (0 if all dry).  Synchronises the stream.
+ */
+int swe_get_state(swe_mesh *mesh, double *h, double *hu, double *hv, double *t, double *dt_next);
+int swe_get_state_device(swe_mesh *mesh, double *d_h, double *d_hu, double *d_hv);
+
+/* Diagnostics (synchronises, copies h to the host). */
+int swe_get_stats(swe_mesh *mesh, swe_stats *stats);
+
+/* perm[p] = caller's cell id stored at internal position p.  host [nt]. */
+int swe_get_permutation(const swe_mesh *mesh, int32_t *perm);
+
+/*
+ * Host tables in caller numbering, for tests of the mesh builder; any pointer may be NULL.
+ *   nbr [nt][3] neighbour cell id, or -tag on a boundary edge
+ *   normal [nt][3][2], length [nt][3], area [nt], inradius [nt], cell_z [nt]
+ */
+int swe_get_tables(const swe_mesh *mesh, int32_t *nbr, double *normal, double *length,
+                   double *area, double *inradius, double *cell_z);
+
+/* Launch facts for reporting: grid, block, loop mode actually in use, kernel launches issued
+ * by this handle so far (step, rate, pack/unpack kernels). */
+int swe_get_launch_info(const swe_mesh *mesh, int32_t *grid, int32_t *block, int32_t *loop_mode,
+                        int64_t *kernel_launches);
+
+const char *swe_last_error(const swe_mesh *mesh);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SWE_B200_H */

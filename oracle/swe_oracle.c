@@ -282,6 +282,9 @@ void oracle_set_state(oracle_mesh *m, const double *h, const double *hu, const d
     memcpy(m->h, h, sizeof(double) * m->nt);
     memcpy(m->hu, hu, sizeof(double) * m->nt);
     memcpy(m->hv, hv, sizeof(double) * m->nt);
+    /* R-15: a dry cell (h <= h_dry) carries no momentum */
+    for (int64_t i = 0; i < m->nt; i++)
+        if (m->h[i] <= m->hdry) { m->hu[i] = 0.0; m->hv[i] = 0.0; }
     m->t = t0; m->dt_valid = 0; m->steps = 0; m->nclamp = 0; m->bnd_volume_out = 0.0L;
 }
 

@@ -1,0 +1,212 @@
+// Host-side mesh builder: orientation, edge matching, geometry, locality renumbering.
+// Input format follows the paper's mesh file (Fig. 4); the renumbering is the
+// single-GPU descendant of the paper's "renumber for contiguous access" idea.
+#include "mesh_builder.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <numeric>
+
+namespace swe {
+
+namespace {
+
+// Hilbert index of (x, y) on a 2^order x 2^order grid (classic rotate-and-flip walk).
+inline uint32_t hilbert_d(uint32_t x, uint32_t y, int order)
+{
+    uint32_t d = 0;
+    for (uint32_t s = 1u << (order - 1); s > 0; s >>= 1) {
+        uint32_t rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
+        d += s * s * ((3u * rx) ^ ry);
+        if (ry == 0) {
+            if (rx == 1) { x = s - 1 - (x & (s - 1)); y = s - 1 - (y & (s - 1)); }
+            else { x &= (s - 1); y &= (s - 1); }
+            std::swap(x, y);
+        } else { x &= (s - 1); y &= (s - 1); }
+    }
+    return d;
+}
+
+void order_hilbert(HostTables &T)
+{
+    const int64_t nt = T.nt;
+    double xmin = T.cx[0], xmax = T.cx[0], ymin = T.cy[0], ymax = T.cy[0];
+    for (int64_t i = 1; i < nt; i++) {
+        xmin = std::min(xmin, T.cx[i]); xmax = std::max(xmax, T.cx[i]);
+        ymin = std::min(ymin, T.cy[i]); ymax = std::max(ymax, T.cy[i]);
+    }
+    const int order = 16;
+    const double ext = std::max(std::max(xmax - xmin, ymax - ymin), 1e-300);
+    const double scale = (double)((1u << order) - 1) / ext; // square curve cells
+    std::vector<uint64_t> key((size_t)nt);
+    for (int64_t i = 0; i < nt; i++) {
+        uint32_t qx = (uint32_t)((T.cx[i] - xmin) * scale), qy = (uint32_t)((T.cy[i] - ymin) * scale);
+        key[(size_t)i] = ((uint64_t)hilbert_d(qx, qy, order) << 32) | (uint64_t)(uint32_t)i;
+    }
+    std::sort(key.begin(), key.end()); // ties broken by caller id: deterministic
+    for (int64_t p = 0; p < nt; p++) T.perm[(size_t)p] = (int32_t)(key[(size_t)p] & 0xffffffffu);
+}
+
+// Reverse Cuthill-McKee on the dual graph (cells adjacent through an edge; degree <= 3).
+void order_rcm(HostTables &T)
+{
+    const int64_t nt = T.nt;
+    std::vector<int32_t> order; order.reserve((size_t)nt);
+    std::vector<uint8_t> seen((size_t)nt, 0);
+    auto degree = [&](int32_t c) {
+        int d = 0;
+        for (int k = 0; k < 3; k++) d += T.nbr[3 * (size_t)c + k] >= 0;
+        return d;
+    };
+    auto bfs = [&](int32_t start, std::vector<int32_t> &out, std::vector<uint8_t> &mark) {
+        size_t head = out.size();
+        out.push_back(start); mark[(size_t)start] = 1;
+        while (head < out.size()) {
+            int32_t c = out[head++];
+            int32_t nb[3]; int n = 0;
+            for (int k = 0; k < 3; k++) {
+                int32_t j = T.nbr[3 * (size_t)c + k];
+                if (j >= 0 && !mark[(size_t)j]) { mark[(size_t)j] = 1; nb[n++] = j; }
+            }
+            std::sort(nb, nb + n, [&](int32_t a, int32_t b) {
+                int da = degree(a), db = degree(b);
+                return da != db ? da < db : a < b;
+            });
+            for (int q = 0; q < n; q++) out.push_back(nb[q]);
+        }
+    };
+    std::vector<uint8_t> tmpmark;
+    for (int64_t s = 0; s < nt; s++) {
+        if (seen[(size_t)s]) continue;
+        // pseudo-peripheral start: last cell of a BFS from s, restricted to s's component
+        tmpmark = seen;
+        std::vector<int32_t> probe;
+        bfs((int32_t)s, probe, tmpmark);
+        int32_t start = probe.back();
+        bfs(start, order, seen);
+    }
+    for (int64_t p = 0; p < nt; p++) T.perm[(size_t)p] = order[(size_t)(nt - 1 - p)];
+}
+
+} // namespace
+
+int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_t nt,
+                 const double *bathymetry, const double *manning, const int8_t *bc_tags,
+                 int ordering, HostTables &T, std::string &err)
+{
+    char msg[256];
+    T.nn = nn; T.nt = nt;
+    try {
+        T.nbr.assign(3 * (size_t)nt, 0);
+        T.normal.resize(6 * (size_t)nt); T.length.resize(3 * (size_t)nt);
+        T.area.resize((size_t)nt); T.inradius.resize((size_t)nt); T.cell_z.resize((size_t)nt);
+        T.manning.resize((size_t)nt); T.cx.resize((size_t)nt); T.cy.resize((size_t)nt);
+        T.perm.resize((size_t)nt); T.inv.resize((size_t)nt);
+    } catch (const std::bad_alloc &) { err = "out of host memory"; return SWE_ERR_NOMEM; }
+
+    for (int64_t i = 0; i < nn; i++) {
+        if (!std::isfinite(nodes_xy[2 * i]) || !std::isfinite(nodes_xy[2 * i + 1]) ||
+            !std::isfinite(bathymetry[i])) {
+            snprintf(msg, sizeof msg, "node %lld has a non-finite coordinate or bed", (long long)i);
+            err = msg; return SWE_ERR_BAD_VALUE;
+        }
+    }
+    // ---- orientation + geometry; vertices after the CCW fix kept for edge matching
+    std::vector<int32_t> vtx(3 * (size_t)nt);
+    std::vector<int8_t> tag(3 * (size_t)nt);
+    for (int64_t i = 0; i < nt; i++) {
+        int32_t v0 = tris[3 * i], v1 = tris[3 * i + 1], v2 = tris[3 * i + 2];
+        int8_t t0 = bc_tags[3 * i], t1 = bc_tags[3 * i + 1], t2 = bc_tags[3 * i + 2];
+        if (v0 < 0 || v0 >= nn || v1 < 0 || v1 >= nn || v2 < 0 || v2 >= nn) {
+            snprintf(msg, sizeof msg, "triangle %lld refers to a node outside [0, %lld)", (long long)i, (long long)nn);
+            err = msg; return SWE_ERR_BAD_INDEX;
+        }
+        if (!(manning[i] >= 0.0) || !std::isfinite(manning[i])) {
+            snprintf(msg, sizeof msg, "cell %lld has a negative or non-finite Manning coefficient", (long long)i);
+            err = msg; return SWE_ERR_BAD_VALUE;
+        }
+        double ax = nodes_xy[2 * (size_t)v0], ay = nodes_xy[2 * (size_t)v0 + 1];
+        double bx = nodes_xy[2 * (size_t)v1], by = nodes_xy[2 * (size_t)v1 + 1];
+        double cx = nodes_xy[2 * (size_t)v2], cy = nodes_xy[2 * (size_t)v2 + 1];
+        double twiceA = (bx - ax) * (cy - ay) - (cx - ax) * (by - ay);
+        if (twiceA < 0.0) { // clockwise: (v0, v2, v1); new edges 0,1,2 are old edges 2,1,0
+            std::swap(v1, v2); std::swap(bx, cx); std::swap(by, cy); std::swap(t0, t2);
+            twiceA = (bx - ax) * (cy - ay) - (cx - ax) * (by - ay);
+        }
+        if (!(twiceA > 0.0)) {
+            snprintf(msg, sizeof msg, "triangle %lld has zero area", (long long)i);
+            err = msg; return SWE_ERR_DEGENERATE;
+        }
+        const double px[4] = { ax, bx, cx, ax }, py[4] = { ay, by, cy, ay };
+        double perimeter = 0.0;
+        for (int k = 0; k < 3; k++) {
+            const double ex = px[k + 1] - px[k], ey = py[k + 1] - py[k];
+            const double L = std::sqrt(ex * ex + ey * ey);
+            T.length[3 * (size_t)i + k] = L;
+            T.normal[6 * (size_t)i + 2 * k] = ey / L;      // CCW triangle: outward = edge rotated by -90 deg
+            T.normal[6 * (size_t)i + 2 * k + 1] = -ex / L;
+            perimeter += L;
+        }
+        const double A = 0.5 * twiceA;
+        T.area[(size_t)i] = A;
+        T.inradius[(size_t)i] = 2.0 * A / perimeter;
+        T.cell_z[(size_t)i] = (bathymetry[v0] + bathymetry[v1] + bathymetry[v2]) / 3.0;
+        T.manning[(size_t)i] = manning[i];
+        T.cx[(size_t)i] = (ax + bx + cx) / 3.0; T.cy[(size_t)i] = (ay + by + cy) / 3.0;
+        vtx[3 * (size_t)i] = v0; vtx[3 * (size_t)i + 1] = v1; vtx[3 * (size_t)i + 2] = v2;
+        tag[3 * (size_t)i] = t0; tag[3 * (size_t)i + 1] = t1; tag[3 * (size_t)i + 2] = t2;
+    }
+    // ---- edge matching: bucket the 3 nt half-edges by their smaller node id (counting sort),
+    //      then pair equal larger ids inside each (tiny) bucket
+    {
+        const size_t ne = 3 * (size_t)nt;
+        std::vector<int64_t> start((size_t)nn + 1, 0);
+        auto lo_of = [&](size_t e) {
+            int32_t a = vtx[e], b = vtx[(e / 3) * 3 + (e % 3 + 1) % 3];
+            return a < b ? a : b;
+        };
+        auto hi_of = [&](size_t e) {
+            int32_t a = vtx[e], b = vtx[(e / 3) * 3 + (e % 3 + 1) % 3];
+            return a < b ? b : a;
+        };
+        for (size_t e = 0; e < ne; e++) start[(size_t)lo_of(e) + 1]++;
+        for (int64_t n = 0; n < nn; n++) start[(size_t)n + 1] += start[(size_t)n];
+        std::vector<int64_t> fill(start.begin(), start.end() - 1);
+        std::vector<int64_t> slot(ne);
+        for (size_t e = 0; e < ne; e++) slot[(size_t)fill[(size_t)lo_of(e)]++] = (int64_t)e;
+        std::fill(T.nbr.begin(), T.nbr.end(), INT32_MIN);
+        for (int64_t n = 0; n < nn; n++) {
+            for (int64_t a = start[(size_t)n]; a < start[(size_t)n + 1]; a++) {
+                const size_t ea = (size_t)slot[(size_t)a];
+                int matches = 0;
+                for (int64_t b = start[(size_t)n]; b < start[(size_t)n + 1]; b++) {
+                    if (b == a) continue;
+                    const size_t eb = (size_t)slot[(size_t)b];
+                    if (hi_of(eb) == hi_of(ea)) {
+                        matches++;
+                        T.nbr[ea] = (int32_t)(eb / 3);
+                    }
+                }
+                if (matches > 1) {
+                    snprintf(msg, sizeof msg, "edge (%d,%d) is shared by more than two triangles", (int)n, (int)hi_of(ea));
+                    err = msg; return SWE_ERR_NON_MANIFOLD;
+                }
+                if (matches == 0) {
+                    int t = tag[ea];
+                    if (t <= 0) t = SWE_BC_WALL; // untagged boundary edge
+                    T.nbr[ea] = -t;
+                    T.inflow_length[t] += T.length[ea];
+                }
+            }
+        }
+    }
+    // ---- locality renumbering of the cells (edge order inside each cell is preserved, R-17)
+    if (ordering == SWE_ORDER_HILBERT) order_hilbert(T);
+    else if (ordering == SWE_ORDER_RCM) order_rcm(T);
+    else std::iota(T.perm.begin(), T.perm.end(), 0);
+    for (int64_t p = 0; p < nt; p++) T.inv[(size_t)T.perm[(size_t)p]] = (int32_t)p;
+    return SWE_OK;
+}
+
+} // namespace swe

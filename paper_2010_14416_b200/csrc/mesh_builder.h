@@ -1,0 +1,34 @@
+// Host-side mesh tables of libswe_b200 (no CUDA here).  See include/swe.h for the contract.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/swe.h"
+
+namespace swe {
+
+// Tables in the CALLER's cell numbering, as built from the paper's mesh format
+// (Fig. 4).  Edge k of cell i joins vertices k and (k+1)%3 after the
+// counter-clockwise fix.
+struct HostTables {
+    int64_t nn = 0, nt = 0;
+    std::vector<int32_t> nbr;     // [nt][3] neighbour cell, or -tag on a boundary edge
+    std::vector<double> normal;   // [nt][3][2] unit outward normal
+    std::vector<double> length;   // [nt][3] L_ij
+    std::vector<double> area;     // [nt] |Omega_i|
+    std::vector<double> inradius; // [nt] R_i
+    std::vector<double> cell_z;   // [nt] cell bed, mean of the node beds (R-1)
+    std::vector<double> manning;  // [nt]
+    std::vector<double> cx, cy;   // [nt] centroids (ordering only)
+    std::vector<int32_t> perm;    // [nt] perm[p] = caller id at internal position p
+    std::vector<int32_t> inv;     // [nt] inverse of perm
+    double inflow_length[SWE_BC_MAX_TAG + 1] = {}; // sum of edge lengths per tag
+};
+
+// Returns SWE_OK or a negative swe_status with a message in err.
+int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_t nt,
+                 const double *bathymetry, const double *manning, const int8_t *bc_tags,
+                 int ordering, HostTables &T, std::string &err);
+
+} // namespace swe

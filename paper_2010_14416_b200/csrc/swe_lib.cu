@@ -1,0 +1,594 @@
+// libswe_b200: C ABI (include/swe.h), kernels and the device-resident time loop.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "mesh_builder.h"
+#include "swe_kernels.cuh"
+
+namespace cg = cooperative_groups;
+using namespace swe;
+
+// =================================================================================================
+// kernels
+// =================================================================================================
+namespace {
+
+constexpr int kDefaultBlock = 256;
+constexpr int kMaxPart = 8192;       // upper bound on the grid of the step kernel
+__device__ __forceinline__ int chunk_count(int nt, int bs) { return (nt + bs - 1) / bs; }
+
+// One time step per launch.  Every block first reduces the per-block maxima of the previous
+// launch into dt (redundantly: a few KB from L2), so no separate finaliser launch and no atomics
+// sit between two steps; block 0 advances the device clock.
+__global__ void __launch_bounds__(kDefaultBlock)
+swe_step_kernel(const Params P, const int cur)
+{
+    __shared__ double s_red[32];
+    const double dt = reduce_dt(P, P.pmax(cur), s_red);
+    const Rec *__restrict__ Uin = P.U(cur);
+    Rec *__restrict__ Uout = P.U(cur ^ 1);
+    double rate = 0.0;
+    unsigned nclamp = 0;
+    const int nchunks = chunk_count(P.nt, blockDim.x);
+    for (int c = blockIdx.x; c < nchunks; c += gridDim.x) {
+        const int i = c * blockDim.x + threadIdx.x;
+        if (i < P.nt) rate = fmax(rate, update_cell<true>(P, Uin, Uout, i, dt, nclamp));
+    }
+    rate = block_max(rate, s_red);
+    if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
+    if (threadIdx.x == 0) {
+        P.pmax(cur ^ 1)[blockIdx.x] = rate;
+        if (blockIdx.x == 0) {
+            Ctrl *c = P.ctrl;
+            c->t += dt; c->dt_last = dt; c->steps += 1;
+            if (!(dt > 0.0)) c->all_dry = 1;
+        }
+    }
+}
+
+// The whole time loop in one cooperative launch: grid barrier between steps instead of a kernel
+// boundary (small meshes are "strictly limited by latencies" of kernel launches).
+__global__ void __launch_bounds__(kDefaultBlock)
+swe_persistent_kernel(const Params P, int cur, const long long nsteps)
+{
+    __shared__ double s_red[32];
+    cg::grid_group grid = cg::this_grid();
+    const int nchunks = chunk_count(P.nt, blockDim.x);
+    for (long long s = 0; s < nsteps; s++) {
+        const double dt = reduce_dt(P, P.pmax(cur), s_red);
+        const Rec *Uin = P.U(cur);
+        Rec *Uout = P.U(cur ^ 1);
+        double rate = 0.0;
+        unsigned nclamp = 0;
+        for (int c = blockIdx.x; c < nchunks; c += gridDim.x) {
+            const int i = c * blockDim.x + threadIdx.x;
+            if (i < P.nt) rate = fmax(rate, update_cell<false>(P, Uin, Uout, i, dt, nclamp));
+        }
+        rate = block_max(rate, s_red);
+        if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);
+        if (threadIdx.x == 0) {
+            P.pmax(cur ^ 1)[blockIdx.x] = rate;
+            if (blockIdx.x == 0) {
+                Ctrl *c = P.ctrl;
+                c->t += dt; c->dt_last = dt; c->steps += 1;
+                if (!(dt > 0.0)) c->all_dry = 1;
+            }
+        }
+        cur ^= 1;
+        grid.sync();
+    }
+}
+
+// Per-block maxima of (sqrt(g h)+|V|)/R for the state in U[cur] (swe_compute_dt, first step).
+__global__ void __launch_bounds__(kDefaultBlock)
+swe_rate_kernel(const Params P, const int cur)
+{
+    __shared__ double s_red[32];
+    double rate = 0.0;
+    const int nchunks = chunk_count(P.nt, blockDim.x);
+    for (int c = blockIdx.x; c < nchunks; c += gridDim.x) {
+        const int i = c * blockDim.x + threadIdx.x;
+        if (i < P.nt) {
+            const Rec U = load_rec<true>(P.U(cur) + i);
+            if (U.h > P.hdry) {
+                const double2 cp = __ldg(P.cellp + i);
+                rate = fmax(rate, (sqrt(P.g * U.h) + sqrt(U.u * U.u + U.v * U.v)) * cp.x);
+            }
+        }
+    }
+    rate = block_max(rate, s_red);
+    if (threadIdx.x == 0) P.pmax(cur)[blockIdx.x] = rate;
+}
+
+// ctrl->dt = CFL / max(pmax[cur]) (for read-back; the step kernels reduce on their own)
+__global__ void swe_finalize_dt_kernel(const Params P, const int cur)
+{
+    __shared__ double s_red[32];
+    const double dt = reduce_dt(P, P.pmax(cur), s_red);
+    if (threadIdx.x == 0) P.ctrl->dt = dt;
+}
+
+// caller numbering (h, hu, hv) -> internal records {h, u, v, z}; dry cells lose their momentum
+__global__ void swe_pack_kernel(const Params P, const int cur, const int32_t *__restrict__ perm,
+                                const double *__restrict__ h, const double *__restrict__ hu,
+                                const double *__restrict__ hv, const double *__restrict__ zcell)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P.nt) return;
+    const int c = perm[p];
+    Rec r; r.h = h[c]; r.z = zcell[p];
+    if (r.h > P.hdry) { r.u = hu[c] / r.h; r.v = hv[c] / r.h; } else { r.u = 0.0; r.v = 0.0; }
+    store_rec(P.U(cur) + p, r);
+}
+__global__ void swe_unpack_kernel(const Params P, const int cur, const int32_t *__restrict__ perm,
+                                  double *__restrict__ h, double *__restrict__ hu, double *__restrict__ hv)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P.nt) return;
+    const int c = perm[p];
+    const Rec r = load_rec<true>(P.U(cur) + p);
+    if (h) h[c] = r.h;
+    if (hu) hu[c] = r.h * r.u;
+    if (hv) hv[c] = r.h * r.v;
+}
+
+} // namespace
+
+// =================================================================================================
+// handle
+// =================================================================================================
+struct swe_mesh {
+    swe_params prm;
+    HostTables T;
+    std::string err;
+    // device
+    bool bound = false, have_state = false, have_rates = false;
+    char *ws = nullptr; size_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;
+    Params P{};
+    int32_t *d_perm = nullptr; double *d_zcell = nullptr; double *d_stage = nullptr;
+    double *d_qn = nullptr;
+    int cur = 0, grid = 0, block = kDefaultBlock, coop_grid = 0, loop_mode = SWE_LOOP_LAUNCH;
+    int64_t launches = 0;
+    double qn_tag[SWE_BC_MAX_TAG + 1] = {};
+    std::map<std::pair<int, int>, cudaGraphExec_t> graphs; // (steps, cur) -> exec
+};
+
+static thread_local std::string g_create_err;
+
+#define CK(call)                                                                         \
+    do {                                                                                 \
+        cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess) {                                                         \
+            m->err = std::string(#call) + ": " + cudaGetErrorString(e_);                 \
+            return SWE_ERR_CUDA;                                                         \
+        }                                                                                \
+    } while (0)
+
+static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+namespace {
+struct Layout {
+    size_t U0, U1, nbr, nrm, coef, cellp, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
+};
+Layout make_layout(int64_t nt)
+{
+    Layout L; size_t o = 0; const size_t n = (size_t)nt;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    L.U0 = take(n * sizeof(Rec)); L.U1 = take(n * sizeof(Rec));
+    L.nbr = take(3 * n * sizeof(int32_t)); L.nrm = take(3 * n * sizeof(double2));
+    L.coef = take(3 * n * sizeof(double)); L.cellp = take(n * sizeof(double2));
+    L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
+    L.stage = take(3 * n * sizeof(double));
+    L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
+    L.qn = take((SWE_BC_MAX_TAG + 1) * sizeof(double)); L.ctrl = take(sizeof(Ctrl));
+    L.total = o;
+    return L;
+}
+} // namespace
+
+extern "C" {
+
+int swe_params_default(swe_params *p)
+{
+    if (!p) return SWE_ERR_INVALID_ARG;
+    p->g = 9.81; p->cfl = 0.9; p->h_dry = 1e-6;
+    p->ordering = SWE_ORDER_HILBERT; p->block_size = 0; p->loop_mode = SWE_LOOP_AUTO; p->reserved = 0;
+    return SWE_OK;
+}
+
+const char *swe_last_error(const swe_mesh *m) { return m ? m->err.c_str() : g_create_err.c_str(); }
+
+int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_t nt,
+                    const double *bathymetry, const double *manning, const int8_t *bc_tags,
+                    const swe_params *params, swe_mesh **out)
+{
+    if (out) *out = nullptr;
+    if (!nodes_xy || !tris || !bathymetry || !manning || !bc_tags || !out || nn <= 0 || nt <= 0 ||
+        nt >= (int64_t)INT32_MAX / 4 || nn >= (int64_t)INT32_MAX) {
+        g_create_err = "swe_mesh_create: NULL pointer or size out of range";
+        return SWE_ERR_INVALID_ARG;
+    }
+    swe_params p;
+    swe_params_default(&p);
+    if (params) p = *params;
+    if (!(p.g > 0.0) || !(p.cfl > 0.0) || !(p.h_dry >= 0.0) || p.ordering < 0 || p.ordering > SWE_ORDER_RCM ||
+        p.loop_mode < 0 || p.loop_mode > SWE_LOOP_LAUNCH ||
+        (p.block_size != 0 && (p.block_size < 64 || p.block_size > kDefaultBlock || p.block_size % 32))) {
+        g_create_err = "swe_mesh_create: invalid swe_params (block_size must be a multiple of 32 in [64, 256])";
+        return SWE_ERR_INVALID_ARG;
+    }
+    swe_mesh *m = new (std::nothrow) swe_mesh();
+    if (!m) { g_create_err = "out of host memory"; return SWE_ERR_NOMEM; }
+    m->prm = p;
+    int rc;
+    try {
+        rc = build_tables(nodes_xy, nn, tris, nt, bathymetry, manning, bc_tags, p.ordering, m->T, m->err);
+    } catch (const std::bad_alloc &) { rc = SWE_ERR_NOMEM; m->err = "out of host memory"; }
+    if (rc != SWE_OK) { g_create_err = m->err; delete m; return rc; }
+    m->block = p.block_size ? p.block_size : kDefaultBlock;
+    *out = m;
+    return SWE_OK;
+}
+
+int swe_mesh_destroy(swe_mesh *m)
+{
+    if (!m) return SWE_OK;
+    for (auto &kv : m->graphs) cudaGraphExecDestroy(kv.second);
+    delete m;
+    return SWE_OK;
+}
+
+int swe_mesh_workspace_bytes(const swe_mesh *m, size_t *bytes)
+{
+    if (!m || !bytes) return SWE_ERR_INVALID_ARG;
+    *bytes = make_layout(m->T.nt).total;
+    return SWE_OK;
+}
+
+int swe_get_permutation(const swe_mesh *m, int32_t *perm)
+{
+    if (!m || !perm) return SWE_ERR_INVALID_ARG;
+    std::memcpy(perm, m->T.perm.data(), sizeof(int32_t) * (size_t)m->T.nt);
+    return SWE_OK;
+}
+
+int swe_get_tables(const swe_mesh *m, int32_t *nbr, double *normal, double *length, double *area,
+                   double *inradius, double *cell_z)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    const size_t n = (size_t)m->T.nt;
+    if (nbr) std::memcpy(nbr, m->T.nbr.data(), 3 * n * sizeof(int32_t));
+    if (normal) std::memcpy(normal, m->T.normal.data(), 6 * n * sizeof(double));
+    if (length) std::memcpy(length, m->T.length.data(), 3 * n * sizeof(double));
+    if (area) std::memcpy(area, m->T.area.data(), n * sizeof(double));
+    if (inradius) std::memcpy(inradius, m->T.inradius.data(), n * sizeof(double));
+    if (cell_z) std::memcpy(cell_z, m->T.cell_z.data(), n * sizeof(double));
+    return SWE_OK;
+}
+
+int swe_get_launch_info(const swe_mesh *m, int32_t *grid, int32_t *block, int32_t *loop_mode, int64_t *launches)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    if (grid) *grid = m->loop_mode == SWE_LOOP_PERSISTENT ? m->coop_grid : m->grid;
+    if (block) *block = m->block;
+    if (loop_mode) *loop_mode = m->loop_mode;
+    if (launches) *launches = m->launches;
+    return SWE_OK;
+}
+
+int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void *cuda_stream)
+{
+    if (!m || !device_workspace) return SWE_ERR_INVALID_ARG;
+    const HostTables &T = m->T;
+    const size_t n = (size_t)T.nt;
+    const Layout L = make_layout(T.nt);
+    if (bytes < L.total || ((uintptr_t)device_workspace & 255u)) {
+        m->err = "workspace too small or not 256-byte aligned";
+        return SWE_ERR_WORKSPACE;
+    }
+    for (auto &kv : m->graphs) cudaGraphExecDestroy(kv.second);
+    m->graphs.clear();
+    m->bound = false; m->have_state = false; m->have_rates = false;
+    m->ws = (char *)device_workspace; m->ws_bytes = bytes; m->stream = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0, coop = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    int occ_step = 0, occ_pers = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_step, swe_step_kernel, m->block, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_pers, swe_persistent_kernel, m->block, 0));
+    if (occ_step < 1 || occ_pers < 1) { m->err = "kernel does not fit on this device"; return SWE_ERR_CUDA; }
+    const int nchunks = (int)((T.nt + m->block - 1) / m->block);
+    // grid: every SM holds its full complement of resident blocks, each walking chunks with a
+    // stride of the grid (a multiple of the SM count); small meshes get one block per chunk
+    m->grid = std::min(std::min(nchunks, sms * occ_step), kMaxPart);
+    m->coop_grid = std::min(std::min(nchunks, sms * occ_pers), kMaxPart);
+    int mode = m->prm.loop_mode;
+    if (mode == SWE_LOOP_AUTO) mode = (coop && nchunks <= 2 * sms * occ_pers) ? SWE_LOOP_PERSISTENT : SWE_LOOP_GRAPH;
+    if (mode == SWE_LOOP_PERSISTENT && !coop) mode = SWE_LOOP_GRAPH;
+    m->loop_mode = mode;
+
+    Params &P = m->P;
+    P.U0 = (Rec *)(m->ws + L.U0); P.U1 = (Rec *)(m->ws + L.U1);
+    P.nbr = (const int32_t *)(m->ws + L.nbr); P.nrm = (const double2 *)(m->ws + L.nrm);
+    P.coef = (const double *)(m->ws + L.coef); P.cellp = (const double2 *)(m->ws + L.cellp);
+    m->d_zcell = (double *)(m->ws + L.zcell); m->d_perm = (int32_t *)(m->ws + L.perm);
+    m->d_stage = (double *)(m->ws + L.stage);
+    P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
+    m->d_qn = (double *)(m->ws + L.qn); P.qn_tag = m->d_qn;
+    P.ctrl = (Ctrl *)(m->ws + L.ctrl);
+    P.nt = (int32_t)T.nt;
+    P.npart = mode == SWE_LOOP_PERSISTENT ? m->coop_grid : m->grid;
+    P.g = m->prm.g; P.cfl = m->prm.cfl; P.hdry = m->prm.h_dry;
+
+    // tables in the internal order, SoA over cells
+    try {
+        std::vector<int32_t> nbr(3 * n);
+        std::vector<double> nrm(6 * n), coef(3 * n), cellp(2 * n), zc(n);
+        for (size_t p = 0; p < n; p++) {
+            const size_t c = (size_t)T.perm[p];
+            for (int k = 0; k < 3; k++) {
+                const int32_t j = T.nbr[3 * c + k];
+                nbr[(size_t)k * n + p] = j >= 0 ? T.inv[(size_t)j] : j;
+                nrm[2 * ((size_t)k * n + p)] = T.normal[6 * c + 2 * k];
+                nrm[2 * ((size_t)k * n + p) + 1] = T.normal[6 * c + 2 * k + 1];
+                coef[(size_t)k * n + p] = T.length[3 * c + k] / T.area[c];
+            }
+            cellp[2 * p] = 1.0 / T.inradius[c];
+            cellp[2 * p + 1] = m->prm.g * T.manning[c] * T.manning[c];
+            zc[p] = T.cell_z[c];
+        }
+        cudaStream_t s = m->stream;
+        CK(cudaMemcpyAsync(m->ws + L.nbr, nbr.data(), 3 * n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.nrm, nrm.data(), 6 * n * sizeof(double), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.coef, coef.data(), 3 * n * sizeof(double), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.cellp, cellp.data(), 2 * n * sizeof(double), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->d_zcell, zc.data(), n * sizeof(double), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->d_perm, T.perm.data(), n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->d_qn, m->qn_tag, sizeof(m->qn_tag), cudaMemcpyHostToDevice, s));
+        CK(cudaMemsetAsync(P.pmax0, 0, kMaxPart * sizeof(double), s));
+        CK(cudaMemsetAsync(P.pmax1, 0, kMaxPart * sizeof(double), s));
+        CK(cudaMemsetAsync(P.ctrl, 0, sizeof(Ctrl), s));
+        CK(cudaStreamSynchronize(s));
+    } catch (const std::bad_alloc &) { m->err = "out of host memory"; return SWE_ERR_NOMEM; }
+    m->bound = true;
+    return SWE_OK;
+}
+
+int swe_set_bc_value(swe_mesh *m, int tag, double total_discharge)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    if (tag < SWE_BC_INFLOW0 || tag > SWE_BC_MAX_TAG || !(m->T.inflow_length[tag] > 0.0)) {
+        m->err = "inflow tag out of range or carried by no boundary edge";
+        return SWE_ERR_BAD_TAG;
+    }
+    if (!std::isfinite(total_discharge)) { m->err = "non-finite discharge"; return SWE_ERR_BAD_VALUE; }
+    m->qn_tag[tag] = -total_discharge / m->T.inflow_length[tag];      // R-20
+    if (m->bound) {
+        CK(cudaMemcpyAsync(m->d_qn, m->qn_tag, sizeof(m->qn_tag), cudaMemcpyHostToDevice, m->stream));
+        CK(cudaStreamSynchronize(m->stream));
+    }
+    return SWE_OK;
+}
+
+static int set_state_common(swe_mesh *m, const double *h, const double *hu, const double *hv, double t0)
+{
+    const int n = (int)m->T.nt;
+    m->cur = 0;
+    swe_pack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_perm, h, hu, hv, m->d_zcell);
+    m->launches++;
+    CK(cudaGetLastError());
+    Ctrl c{}; c.t = t0;
+    CK(cudaMemcpyAsync(m->P.ctrl, &c, sizeof(Ctrl), cudaMemcpyHostToDevice, m->stream));
+    CK(cudaStreamSynchronize(m->stream));
+    m->have_state = true; m->have_rates = false;
+    return SWE_OK;
+}
+
+int swe_set_state(swe_mesh *m, const double *h, const double *hu, const double *hv, double t0)
+{
+    if (!m || !h || !hu || !hv || !std::isfinite(t0)) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    const size_t n = (size_t)m->T.nt;
+    for (size_t i = 0; i < n; i++) {
+        if (!(h[i] >= 0.0) || !std::isfinite(h[i]) || !std::isfinite(hu[i]) || !std::isfinite(hv[i])) {
+            m->err = "state has a negative depth or a non-finite value at cell " + std::to_string(i);
+            return SWE_ERR_BAD_VALUE;
+        }
+    }
+    double *st = m->d_stage;
+    CK(cudaMemcpyAsync(st, h, n * sizeof(double), cudaMemcpyHostToDevice, m->stream));
+    CK(cudaMemcpyAsync(st + n, hu, n * sizeof(double), cudaMemcpyHostToDevice, m->stream));
+    CK(cudaMemcpyAsync(st + 2 * n, hv, n * sizeof(double), cudaMemcpyHostToDevice, m->stream));
+    return set_state_common(m, st, st + n, st + 2 * n, t0);
+}
+
+int swe_set_state_device(swe_mesh *m, const double *d_h, const double *d_hu, const double *d_hv, double t0)
+{
+    if (!m || !d_h || !d_hu || !d_hv || !std::isfinite(t0)) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    return set_state_common(m, d_h, d_hu, d_hv, t0);
+}
+
+static int ensure_rates(swe_mesh *m)
+{
+    if (m->have_rates) return SWE_OK;
+    swe_rate_kernel<<<m->P.npart, m->block, 0, m->stream>>>(m->P, m->cur);
+    m->launches++;
+    CK(cudaGetLastError());
+    m->have_rates = true;
+    return SWE_OK;
+}
+
+static int read_ctrl(swe_mesh *m, Ctrl *c, bool finalize)
+{
+    if (finalize) {
+        int rc = ensure_rates(m);
+        if (rc != SWE_OK) return rc;
+        swe_finalize_dt_kernel<<<1, 256, 0, m->stream>>>(m->P, m->cur);
+        m->launches++;
+        CK(cudaGetLastError());
+    }
+    CK(cudaMemcpyAsync(c, m->P.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, m->stream));
+    CK(cudaStreamSynchronize(m->stream));
+    return SWE_OK;
+}
+
+int swe_compute_dt(swe_mesh *m, double *dt_out)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
+    m->have_rates = false;      // recompute from the current state, as documented
+    Ctrl c;
+    int rc = read_ctrl(m, &c, true);
+    if (rc != SWE_OK) return rc;
+    if (dt_out) *dt_out = c.dt;
+    if (!(c.dt > 0.0)) { m->err = "every cell is dry"; return SWE_ERR_ALL_DRY; }
+    return SWE_OK;
+}
+
+static int launch_steps_direct(swe_mesh *m, int64_t n)
+{
+    for (int64_t s = 0; s < n; s++) {
+        swe_step_kernel<<<m->grid, m->block, 0, m->stream>>>(m->P, m->cur);
+        m->cur ^= 1;
+        m->launches++;
+    }
+    CK(cudaGetLastError());
+    return SWE_OK;
+}
+
+static int graph_for(swe_mesh *m, int steps, cudaGraphExec_t *out)
+{
+    auto key = std::make_pair(steps, m->cur);
+    auto it = m->graphs.find(key);
+    if (it != m->graphs.end()) { *out = it->second; return SWE_OK; }
+    cudaGraph_t g = nullptr; cudaGraphExec_t ex = nullptr;
+    // capture on a private stream so that a NULL (legacy default) user stream works too
+    cudaStream_t cap;
+    CK(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+    int c = m->cur;
+    if (e == cudaSuccess) {
+        for (int s = 0; s < steps; s++) { swe_step_kernel<<<m->grid, m->block, 0, cap>>>(m->P, c); c ^= 1; }
+        e = cudaStreamEndCapture(cap, &g);
+    }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&ex, g, 0);
+    if (g) cudaGraphDestroy(g);
+    cudaStreamDestroy(cap);
+    if (e != cudaSuccess) { m->err = std::string("CUDA graph build: ") + cudaGetErrorString(e); return SWE_ERR_CUDA; }
+    m->graphs[key] = ex;
+    *out = ex;
+    return SWE_OK;
+}
+
+int swe_run(swe_mesh *m, int64_t nsteps)
+{
+    if (!m || nsteps < 0) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
+    if (nsteps == 0) return SWE_OK;
+    int rc = ensure_rates(m);
+    if (rc != SWE_OK) return rc;
+    if (m->loop_mode == SWE_LOOP_PERSISTENT) {
+        Params P = m->P; int cur = m->cur; long long ns = nsteps;
+        void *args[] = { &P, &cur, &ns };
+        CK(cudaLaunchCooperativeKernel((void *)swe_persistent_kernel, dim3(m->coop_grid), dim3(m->block), args, 0, m->stream));
+        m->launches++;
+        m->cur ^= (int)(nsteps & 1);
+        return SWE_OK;
+    }
+    if (m->loop_mode == SWE_LOOP_LAUNCH) return launch_steps_direct(m, nsteps);
+    // CUDA graphs of 128 / 16 / 2 steps (even, so the ping-pong parity is unchanged), rest direct
+    static const int chunks[3] = { 128, 16, 2 };
+    int64_t left = nsteps;
+    for (int q = 0; q < 3; q++) {
+        while (left >= chunks[q]) {
+            cudaGraphExec_t ex;
+            rc = graph_for(m, chunks[q], &ex);
+            if (rc != SWE_OK) return rc;
+            CK(cudaGraphLaunch(ex, m->stream));
+            m->launches += chunks[q];
+            left -= chunks[q];
+        }
+    }
+    return launch_steps_direct(m, left);
+}
+
+int swe_step(swe_mesh *m) { return swe_run(m, 1); }
+
+int swe_sync(swe_mesh *m)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    CK(cudaStreamSynchronize(m->stream));
+    return SWE_OK;
+}
+
+int swe_get_state_device(swe_mesh *m, double *d_h, double *d_hu, double *d_hv)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
+    const int n = (int)m->T.nt;
+    swe_unpack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, m->cur, m->d_perm, d_h, d_hu, d_hv);
+    m->launches++;
+    CK(cudaGetLastError());
+    return SWE_OK;
+}
+
+int swe_get_state(swe_mesh *m, double *h, double *hu, double *hv, double *t, double *dt_next)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
+    const size_t n = (size_t)m->T.nt;
+    double *st = m->d_stage;
+    if (h || hu || hv) {
+        int rc = swe_get_state_device(m, h ? st : nullptr, hu ? st + n : nullptr, hv ? st + 2 * n : nullptr);
+        if (rc != SWE_OK) return rc;
+        if (h) CK(cudaMemcpyAsync(h, st, n * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+        if (hu) CK(cudaMemcpyAsync(hu, st + n, n * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+        if (hv) CK(cudaMemcpyAsync(hv, st + 2 * n, n * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+    }
+    Ctrl c;
+    int rc = read_ctrl(m, &c, dt_next != nullptr);
+    if (rc != SWE_OK) return rc;
+    if (t) *t = c.t;
+    if (dt_next) *dt_next = c.dt;
+    return SWE_OK;
+}
+
+int swe_get_stats(swe_mesh *m, swe_stats *s)
+{
+    if (!m || !s) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
+    const size_t n = (size_t)m->T.nt;
+    std::vector<double> h(n), hu(n), hv(n);
+    double t = 0;
+    int rc = swe_get_state(m, h.data(), hu.data(), hv.data(), &t, nullptr);
+    if (rc != SWE_OK) return rc;
+    Ctrl c;
+    rc = read_ctrl(m, &c, false);
+    if (rc != SWE_OK) return rc;
+    long double vol = 0.0L; int64_t ndry = 0, nbad = 0;
+    for (size_t i = 0; i < n; i++) {
+        vol += (long double)h[i] * (long double)m->T.area[i];
+        ndry += h[i] <= m->prm.h_dry;
+        nbad += !(std::isfinite(h[i]) && std::isfinite(hu[i]) && std::isfinite(hv[i]));
+    }
+    s->volume = (double)vol; s->t = c.t; s->dt_last = c.dt_last; s->steps = c.steps;
+    s->n_dry = ndry; s->n_clamped = (int64_t)c.n_clamped; s->n_nonfinite = nbad;
+    return SWE_OK;
+}
+
+} // extern "C"

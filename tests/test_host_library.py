@@ -1,0 +1,130 @@
+"""CPU-only checks of the C-ABI library: it loads, exports every declared symbol, and its host
+mesh builder (no CUDA involved) agrees with the oracle's independent geometry."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle.swe_oracle import OracleSolver
+from paper_2010_14416_b200 import binding as B
+from paper_2010_14416_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    L = B.load_library()
+    header = open(os.path.join(ROOT, "include", "swe.h")).read()
+    declared = set(re.findall(r"\b(swe_[a-z_]+)\s*\(", header))
+    declared -= {"swe_last_error"} - set(B.SYMBOLS)
+    assert declared == set(B.SYMBOLS)
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_struct_sizes_match_header():
+    assert ctypes.sizeof(B.SweParams) == 3 * 8 + 4 * 4
+    assert ctypes.sizeof(B.SweStats) == 3 * 8 + 4 * 8
+    p = B.SweParams()
+    B.load_library().swe_params_default(ctypes.byref(p))
+    assert (p.g, p.cfl, p.h_dry, p.ordering, p.loop_mode) == (9.81, 0.9, 1e-6, B.ORDER_HILBERT, B.LOOP_AUTO)
+
+
+@pytest.mark.parametrize("ordering", [B.ORDER_IDENTITY, B.ORDER_HILBERT, B.ORDER_RCM])
+def test_tables_match_oracle_geometry(ordering):
+    w = W.config4(nx=60, ny=15)
+    m = B.SweMesh.from_workload(w, ordering=ordering)
+    t = m.get_tables()
+    geo = OracleSolver.from_workload(w).geometry()
+    nbr_o = geo["nbr"].copy()
+    bnd = nbr_o < 0
+    assert ((t["nbr"] < 0) == bnd).all()
+    np.testing.assert_array_equal(t["nbr"][~bnd], nbr_o[~bnd])
+    # boundary edges carry -tag
+    np.testing.assert_array_equal(-t["nbr"][bnd], np.maximum(w.bc_tags[bnd], 1))
+    np.testing.assert_allclose(t["normal"][:, :, 0], geo["n1"], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(t["normal"][:, :, 1], geo["n2"], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(t["length"], geo["len"], rtol=1e-15)
+    np.testing.assert_allclose(t["area"], geo["area"], rtol=1e-15)
+    np.testing.assert_allclose(t["inradius"], geo["rin"], rtol=1e-15)
+    np.testing.assert_allclose(t["cell_z"], geo["z"], rtol=1e-15, atol=1e-15)
+    perm = m.get_permutation()
+    assert sorted(perm.tolist()) == list(range(w.ncells))
+    if ordering == B.ORDER_IDENTITY:
+        assert (perm == np.arange(w.ncells)).all()
+
+
+def _mean_neighbour_distance(w, perm):
+    inv = np.empty_like(perm)
+    inv[perm] = np.arange(perm.size, dtype=perm.dtype)
+    nbr = OracleSolver.from_workload(w).geometry()["nbr"]
+    i = np.repeat(np.arange(w.ncells), 3)
+    j = nbr.ravel()
+    ok = j >= 0
+    return np.abs(inv[i[ok]].astype(np.int64) - inv[j[ok]].astype(np.int64)).mean()
+
+
+def test_locality_orderings_shrink_neighbour_distance():
+    """a13: the Hilbert / RCM numbering keeps a cell's neighbours close in memory."""
+    w = W.config2(nx=200, ny=20)
+    d_id = _mean_neighbour_distance(w, np.arange(w.ncells, dtype=np.int32))
+    d_h = _mean_neighbour_distance(w, B.SweMesh.from_workload(w, ordering=B.ORDER_HILBERT).get_permutation())
+    d_r = _mean_neighbour_distance(w, B.SweMesh.from_workload(w, ordering=B.ORDER_RCM).get_permutation())
+    assert d_id > 1000          # the generator's random permutation scatters neighbours
+    assert d_h < 40 and d_r < 80
+
+
+def test_clockwise_triangles_and_tag_permutation():
+    w = W.config4(nx=40, ny=10)
+    tris, tags = w.tris.copy(), w.bc_tags.copy()
+    flip = np.arange(w.ncells) % 2 == 0
+    tris[flip] = tris[flip][:, [0, 2, 1]]
+    tags[flip] = tags[flip][:, [2, 1, 0]]
+    a = B.SweMesh(w.nodes_xy, w.tris, w.bathymetry, w.manning, w.bc_tags).get_tables()
+    b = B.SweMesh(w.nodes_xy, tris, w.bathymetry, w.manning, tags).get_tables()
+    # an unflipped cell is unchanged; a flipped cell (v0,v2,v1) is re-oriented to (v0,v1,v2)
+    for key in ("nbr", "length", "area", "inradius"):
+        np.testing.assert_array_equal(a[key], b[key])
+
+
+def test_invalid_input_codes():
+    w = W.two_triangles()
+    bad = w.tris.copy(); bad[0, 0] = 9
+    with pytest.raises(B.SweError) as e:
+        B.SweMesh(w.nodes_xy, bad, w.bathymetry, w.manning, w.bc_tags)
+    assert e.value.code == -2
+    deg = w.tris.copy(); deg[0] = [0, 1, 1]
+    with pytest.raises(B.SweError) as e:
+        B.SweMesh(w.nodes_xy, deg, w.bathymetry, w.manning, w.bc_tags)
+    assert e.value.code == -3
+    tri3 = np.vstack([w.tris, [[0, 2, 1]]]).astype(np.int32)
+    with pytest.raises(B.SweError) as e:
+        B.SweMesh(w.nodes_xy, tri3, w.bathymetry, np.zeros(3), np.ones((3, 3), dtype=np.int8))
+    assert e.value.code == -4
+    with pytest.raises(B.SweError) as e:
+        B.SweMesh(w.nodes_xy, w.tris, w.bathymetry, np.array([0.0, -1.0]), w.bc_tags)
+    assert e.value.code == -5
+    xy = w.nodes_xy.copy(); xy[1, 0] = np.nan
+    with pytest.raises(B.SweError) as e:
+        B.SweMesh(xy, w.tris, w.bathymetry, w.manning, w.bc_tags)
+    assert e.value.code == -5
+    with pytest.raises(B.SweError) as e:
+        B.SweMesh(w.nodes_xy, w.tris, w.bathymetry, w.manning, w.bc_tags, block_size=100)
+    assert e.value.code == -1
+
+
+def test_compute_entry_points_fail_loudly_without_a_device():
+    """No CPU fallback: unbound handles refuse to compute."""
+    w = W.two_triangles()
+    m = B.SweMesh.from_workload(w)
+    assert m.workspace_bytes() > 0
+    for call in (lambda: m.set_state(w.h, w.hu, w.hv), m.compute_dt, m.step, lambda: m.run(3),
+                 m.get_state, m.get_stats, m.sync):
+        with pytest.raises(B.SweError) as e:
+            call()
+        assert e.value.code == -6
+    with pytest.raises(B.SweError) as e:
+        m.set_bc_value(3, 1.0)       # no edge carries tag 3 on this mesh
+    assert e.value.code == -11
