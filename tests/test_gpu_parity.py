@@ -1,0 +1,191 @@
+"""GPU-vs-oracle parity through the C ABI (north_star tolerances, written here):
+
+  |x_gpu - x_oracle| <= 1e-10 + 1e-10 |x_oracle|   for h, hu, hv after the stated steps
+  dt matched to 1e-12 relative, simulated time likewise
+  dry-cell mask (h <= h_dry) identical
+
+Both sides get the same seeded arrays from paper_2010_14416_b200.workloads.
+"""
+import numpy as np
+import pytest
+
+from oracle.swe_oracle import OracleSolver
+from paper_2010_14416_b200 import binding as B
+from paper_2010_14416_b200 import workloads as W
+from tests.analytic import stoker_profile
+
+pytestmark = pytest.mark.gpu
+
+RTOL = ATOL = 1e-10
+
+
+def run_both(w, nsteps, **kw):
+    m = B.SweMesh.from_workload(w, **kw).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    o = OracleSolver.from_workload(w)
+    dt0_g, dt0_o = m.compute_dt(), o.compute_dt()
+    assert dt0_g == pytest.approx(dt0_o, rel=1e-12)
+    m.run(nsteps)
+    done = o.run(nsteps)
+    assert done == nsteps
+    return m, o
+
+
+def assert_parity(m, o, w):
+    hg, hug, hvg, tg, dtg = m.get_state()
+    ho, huo, hvo, to, dto = o.get_state()
+    np.testing.assert_array_equal(hg <= w.h_dry, ho <= w.h_dry)
+    np.testing.assert_allclose(hg, ho, rtol=RTOL, atol=ATOL)
+    np.testing.assert_allclose(hug, huo, rtol=RTOL, atol=ATOL)
+    np.testing.assert_allclose(hvg, hvo, rtol=RTOL, atol=ATOL)
+    assert tg == pytest.approx(to, rel=1e-12)
+    assert dtg == pytest.approx(dto, rel=1e-12)
+    sg, so = m.get_stats(), o.stats()
+    assert sg["n_clamped"] == 0 and so["nclamp"] == 0 and sg["n_nonfinite"] == 0
+    assert sg["n_dry"] == so["ndry"]
+    assert sg["volume"] == pytest.approx(so["volume"], rel=1e-12)
+    assert sg["steps"] == so["steps"]
+    return hg, hug, hvg, tg
+
+
+LOOPS = [B.LOOP_GRAPH, B.LOOP_PERSISTENT, B.LOOP_LAUNCH]
+
+
+@pytest.mark.parametrize("loop_mode", LOOPS)
+def test_config1_wetwet_dambreak(loop_mode):
+    """BASELINE configs[0] in full: 2000 cells, 500 steps, every loop mode."""
+    w = W.config1()
+    m, o = run_both(w, w.nsteps, loop_mode=loop_mode)
+    h, hu, hv, t = assert_parity(m, o, w)
+    assert m.get_launch_info()["loop_mode"] == B.LOOP_NAMES[loop_mode]
+    v0 = float(np.sum(w.h * OracleSolver.from_workload(w).geometry()["area"]))
+    assert m.get_stats()["volume"] == pytest.approx(v0, rel=1e-12)
+
+
+def test_config1_stoker_profile():
+    """The GPU result itself against the closed-form Stoker solution before wall reflection."""
+    w = W.config1()
+    m = B.SweMesh.from_workload(w).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    while True:
+        m.run(20)
+        h, hu, hv, t, _ = m.get_state()
+        if t >= 8.0:
+            break
+    cx = W.centroids(w.nodes_xy, w.tris)[:, 0]
+    hex_, _ = stoker_profile((cx - 50.0) / t, 1.0, 0.5)
+    area = m.get_tables()["area"]
+    assert float(np.sum(np.abs(h - hex_) * area) / area.sum()) < 0.012
+
+
+@pytest.mark.parametrize("ordering", [B.ORDER_IDENTITY, B.ORDER_HILBERT, B.ORDER_RCM])
+def test_config2_wetdry_dambreak_full(ordering):
+    """BASELINE configs[1] in full: 200k cells, Manning 0.03, wet/dry front, 2000 steps."""
+    w = W.config2()
+    m, o = run_both(w, w.nsteps, ordering=ordering)
+    assert_parity(m, o, w)
+
+
+def test_config3_lake_at_rest_reduced_full_steps():
+    """configs[2] shape (bumps, islands, Manning 0.025) at 400x200 squares, all 1000 steps."""
+    w = W.config3(nx=400, ny=200)
+    m, o = run_both(w, 1000)
+    h, hu, hv, _ = assert_parity(m, o, w)
+    z = m.get_tables()["cell_z"]
+    wet = h > w.h_dry
+    np.testing.assert_array_equal(~wet, w.h <= w.h_dry)
+    assert np.abs(h[wet] + z[wet] - 2.0).max() < 1e-12
+    assert np.abs(hu[wet] / h[wet]).max() < 1e-10 and np.abs(hv[wet] / h[wet]).max() < 1e-10
+
+
+def test_config4_river_reduced_full_steps():
+    """configs[3] shape (channel, noise terrain, varying Manning, inflow/outflow) at 640x160."""
+    w = W.config4(nx=640, ny=160)
+    m, o = run_both(w, 2000)
+    assert_parity(m, o, w)
+    st, so = m.get_stats(), o.stats()
+    v0 = float(np.sum(w.h * m.get_tables()["area"]))
+    # mass balance against the oracle's boundary-flux integral (R-20)
+    assert st["volume"] - v0 == pytest.approx(-so["boundary_volume_out"], rel=1e-8)
+
+
+def test_ordering_invariance_bitwise():
+    """R-17: renumbering permutes cells only, so results agree bit for bit in caller numbering."""
+    w = W.config4(nx=200, ny=50)
+    out = []
+    for ordering in (B.ORDER_IDENTITY, B.ORDER_HILBERT, B.ORDER_RCM):
+        m = B.SweMesh.from_workload(w, ordering=ordering, loop_mode=B.LOOP_GRAPH).bind_device()
+        m.set_state(w.h, w.hu, w.hv)
+        m.run(300)
+        out.append(m.get_state())
+    for other in out[1:]:
+        for a, b in zip(out[0][:3], other[:3]):
+            np.testing.assert_array_equal(a, b)
+        assert out[0][3] == other[3] and out[0][4] == other[4]
+
+
+def test_determinism_and_loop_modes_bitwise():
+    """Two runs, and the three loop modes, give identical bits (no atomics in the data path)."""
+    w = W.config2(nx=300, ny=30)
+    ref = None
+    for loop_mode in (B.LOOP_GRAPH, B.LOOP_GRAPH, B.LOOP_PERSISTENT, B.LOOP_LAUNCH):
+        m = B.SweMesh.from_workload(w, loop_mode=loop_mode).bind_device()
+        m.set_state(w.h, w.hu, w.hv)
+        m.run(137)
+        m.run(64)
+        m.step()
+        got = m.get_state()
+        if ref is None:
+            ref = got
+        else:
+            for a, b in zip(ref[:3], got[:3]):
+                np.testing.assert_array_equal(a, b)
+            assert ref[3] == got[3] and ref[4] == got[4]
+
+
+def test_edge_cases():
+    # all dry: no time step, state unchanged, error code from compute_dt
+    w = W.canal_dam_break(10, 3, h_left=0.0, h_right=0.0, length=10.0)
+    m = B.SweMesh.from_workload(w).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    with pytest.raises(B.SweError) as e:
+        m.compute_dt()
+    assert e.value.code == B.ERR_ALL_DRY
+    m.run(3)
+    h, hu, hv, t, dt = m.get_state()
+    assert (h == 0).all() and t == 0.0 and dt == 0.0
+    # two cells (the smallest mesh), ragged tail of one partial warp
+    w = W.two_triangles()
+    m, o = run_both(w, 25)
+    assert_parity(m, o, w)
+    # a mesh size that is not a multiple of the block size, several blocks, tiny block size
+    w = W.canal_dam_break(37, 7, seed=9, length=37.0, manning=0.02, h_right=0.0)
+    m, o = run_both(w, 200, block_size=64)
+    assert_parity(m, o, w)
+    # state with momentum in dry cells is sanitised identically on both sides (R-15)
+    w = W.canal_dam_break(20, 4, seed=4, length=20.0, h_right=5e-7)
+    w.hu[:] = 0.01
+    m, o = run_both(w, 30)
+    assert_parity(m, o, w)
+    # invalid state is rejected
+    bad = w.h.copy(); bad[3] = -1.0
+    with pytest.raises(B.SweError) as e:
+        m.set_state(bad, w.hu, w.hv)
+    assert e.value.code == -5
+
+
+def test_device_state_roundtrip():
+    import torch
+    w = W.config1()
+    m = B.SweMesh.from_workload(w).bind_device()
+    with torch.cuda.stream(m.stream):
+        d = [torch.from_numpy(x.copy()).cuda() for x in (w.h, w.hu, w.hv)]
+        m.set_state_device(*d)
+        m.run(10)
+        out = [torch.empty(w.ncells, dtype=torch.float64, device="cuda") for _ in range(3)]
+        m.get_state_device(*out)
+    m.sync()
+    h, hu, hv, _, _ = m.get_state()
+    np.testing.assert_array_equal(out[0].cpu().numpy(), h)
+    np.testing.assert_array_equal(out[1].cpu().numpy(), hu)
+    np.testing.assert_array_equal(out[2].cpu().numpy(), hv)
