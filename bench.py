@@ -1,0 +1,297 @@
+#!/usr/bin/env python
+"""bench.py -- SWE FP64 cell-updates/s on B200 (BASELINE.json metric) + HBM roofline fraction.
+
+A "step" is one pass of the whole hot path (gather, reconstruction, HLLC
+fluxes, sources, friction, update, CFL reduction) over the whole mesh = one solver time step.
+Default workload: BASELINE.json configs[3] (river, 13,005,000 cells) -- the largest single-GPU
+config and one of the ">= 4M-cell meshes" the north_star's roofline target is quoted on; its
+2.5 GB of device data are far larger than the 126 MB L2, so no L2 flush is needed between steps.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+N > 1 (torchrun): the path does not shard ("replicas only"): every rank runs the same
+workload independently, value = all ranks' cell-updates / max-over-ranks device time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2010_14416_b200 import workloads as W  # noqa: E402
+
+ALGO_BYTES_PER_CELL = 156.0   # 132 B read + 24 B written per cell-update
+METRIC = "SWE FP64 cell-updates/s"
+UNIT = "cell-updates/s"
+
+
+def make_workload(name: str):
+    if name == "config1":
+        return W.config1()
+    if name == "config2":
+        return W.config2()
+    if name == "config3":
+        return W.config3()
+    if name == "config4":
+        return W.config4()
+    if name.startswith("sweep_"):
+        return W.config5(name[len("sweep_"):])
+    raise SystemExit(f"unknown workload {name}")
+
+
+def make_sample(name: str):
+    """Bounded sample of the same workload for the CPU oracle: same recipe, fewer squares."""
+    if name == "config4":
+        return W.config4(nx=1275, ny=319), "config4 recipe at 1275x319 squares (813,450 cells)"
+    if name == "config3":
+        return W.config3(nx=1000, ny=500), "config3 recipe at 1000x500 squares (1,000,000 cells)"
+    if name.startswith("sweep_") and W.SWEEP_NY[name[6:]] > 316:
+        return W.config5("0.5M"), "config5 recipe at 0.5M cells"
+    return make_workload(name), "the full workload"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_traffic(workload: str):
+    """dram bytes per launch of the step kernel from the committed ncu --set full capture."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(workload)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for ts, r in self.rows if t0 - 0.05 <= ts <= t1 + 0.15 and len(r) >= 7] or \
+               [r for _, r in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                "samples": len(rows), "power_w_max": max(float(r[2]) for r in rows)}
+
+
+def time_oracle(w, steps: int, warmup: int, threads=None):
+    """The oracle as it stands on the host cores: returns (cell-updates/s, threads used)."""
+    from oracle.swe_oracle import OracleSolver
+    o = OracleSolver.from_workload(w)
+    if threads is None:   # pick the thread count that is actually fastest on this box
+        best = (0.0, 1)
+        for n in sorted({1, 2, 4, 8, 16, 32, os.cpu_count() or 1}):
+            if n > (os.cpu_count() or 1):
+                continue
+            o.set_threads(n)
+            o.compute_dt()
+            o.run(1)                       # spin the thread team up
+            t0 = time.perf_counter()
+            o.run(3)
+            r = 3 * w.ncells / (time.perf_counter() - t0)
+            if r > best[0]:
+                best = (r, n)
+        threads = best[1]
+        o.set_state(w.h, w.hu, w.hv)
+    o.set_threads(threads)
+    o.compute_dt()
+    o.run(warmup)
+    t0 = time.perf_counter()
+    done = o.run(steps)
+    dt = time.perf_counter() - t0
+    return done * w.ncells / dt, threads, dt
+
+
+def run_reference(args, rank: int, world: int):
+    """--impl reference: the oracle, as it stands, on the box's host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    sample, what = make_sample(args.workload)
+    steps = max(1, min(args.steps, 20))
+    value, threads, secs = time_oracle(sample, steps, min(args.warmup, 3))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": min(args.warmup, 3), "ms_per_step": 1e3 * secs / steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": args.workload, "sample": what},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": what},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_gpu(args, rank: int, world: int, local_rank: int):
+    import torch
+    import torch.distributed as dist
+    from paper_2010_14416_b200 import binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: CUDA is not available and there is no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = f"cuda:{local_rank}"
+
+    w = make_workload(args.workload)
+    n = w.ncells
+    order = {"hilbert": B.ORDER_HILBERT, "rcm": B.ORDER_RCM, "identity": B.ORDER_IDENTITY}[args.ordering]
+    loop = {"auto": B.LOOP_AUTO, "graph": B.LOOP_GRAPH, "persistent": B.LOOP_PERSISTENT,
+            "launch": B.LOOP_LAUNCH}[args.loop]
+    t_build = time.perf_counter()
+    m = B.SweMesh.from_workload(w, ordering=order, loop_mode=loop).bind_device(dev)
+    t_build = time.perf_counter() - t_build
+    # pinned host buffers for the end-to-end leg
+    pin = [torch.empty(n, dtype=torch.float64).pin_memory() for _ in range(6)]
+    hin = [p.numpy() for p in pin[:3]]
+    hout = [p.numpy() for p in pin[3:]]
+    for dst, src in zip(hin, (w.h, w.hu, w.hv)):
+        dst[:] = src
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident leg: W warm-up steps, then exactly K timed steps in one swe_run ----
+    m.set_state(*hin)
+    m.run(args.warmup)
+    m.sync()
+    launches0 = m.get_launch_info()["kernel_launches"]
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.time()
+    ev0.record(m.stream)
+    m.run(args.steps)
+    ev1.record(m.stream)
+    barrier()
+    t1 = time.time()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop(t0, t1)
+    info = m.get_launch_info()
+    launches = info["kernel_launches"] - launches0
+    stats = m.get_stats()
+
+    # ---- end-to-end leg through the C ABI with host buffers: set_state + run(K) + get_state ----
+    barrier()
+    e0 = time.perf_counter()
+    m.set_state(*hin)
+    m.run(args.steps)
+    m.get_state_into(*hout)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - e0
+
+    times = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    ms, e2e_ms = times.tolist()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    total_updates = float(n) * args.steps * world
+    value = total_updates / (ms * 1e-3)
+    peak, peak_src = load_peaks()
+    kernel_ms = ms / args.steps                       # one step kernel launch per step
+    achieved = ALGO_BYTES_PER_CELL * n / (kernel_ms * 1e-3) / 1e9
+    sample, what = make_sample(args.workload)
+    cpu_value, cpu_threads, _ = time_oracle(sample, 10 if sample.ncells > 300000 else 100, 2)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "name": w.name, "cells": n, "nodes": w.nnodes,
+                   "ordering": args.ordering, "loop_mode": info["loop_mode"],
+                   "grid": info["grid"], "block": info["block"],
+                   "l2_policy": "inputs larger than L2 (no flush)" if n * 164 > 2 * 126e6
+                   else "working set fits in L2; a time loop re-reads its own output, no flush",
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "mesh_build_s": round(t_build, 2), "wet_fraction_end": 1.0 - stats["n_dry"] / n,
+                   "n_clamped": stats["n_clamped"]},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": load_traffic(args.workload),
+                     "kernel": "swe_step_kernel", "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
+                     "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
+        "cpu_baseline": {"value": cpu_value, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
+                         "sample": what},
+        "e2e": {"value": total_updates / (e2e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": 24.0 * n / args.steps, "d2h_bytes_per_step": 24.0 * n / args.steps,
+                "job": "swe_set_state(pinned host) + swe_run(K) + swe_get_state(pinned host); "
+                       "bytes are per job / K"},
+        "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--workload", default="config4")
+    ap.add_argument("--ordering", default="hilbert", choices=["hilbert", "rcm", "identity"])
+    ap.add_argument("--loop", default="auto", choices=["auto", "graph", "persistent", "launch"])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_gpu(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
