@@ -26,6 +26,23 @@ struct HostTables {
     double inflow_length[SWE_BC_MAX_TAG + 1] = {}; // sum of edge lengths per tag
 };
 
+// Tile tables of the step kernel (swe_kernels.cuh), in the INTERNAL cell numbering: the cells
+// are cut into tiles of tile_cells consecutive cells; every edge that touches a tile appears
+// once in that tile's edge list (an edge between two tiles appears in both lists).
+struct HostEdge { int32_t a, b; double n1, n2, len; };                          // 32 bytes
+struct HostCell { uint32_t slots01, slots2; double inv_area, inv_R, gm2; };     // 32 bytes
+struct TileTables {
+    int32_t tile_cells = 0;
+    int64_t ntiles = 0;
+    int32_t max_edges = 0;             // longest edge list of any tile
+    std::vector<int32_t> estart;       // [ntiles + 1] offsets into edges
+    std::vector<HostEdge> edges;
+    std::vector<HostCell> cells;       // [nt]
+};
+
+// Returns SWE_OK or a negative swe_status with a message in err.
+int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, std::string &err);
+
 // Returns SWE_OK or a negative swe_status with a message in err.
 int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_t nt,
                  const double *bathymetry, const double *manning, const int8_t *bc_tags,

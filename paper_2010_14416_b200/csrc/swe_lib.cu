@@ -19,14 +19,19 @@ using namespace swe;
 // =================================================================================================
 namespace {
 
-constexpr int kDefaultBlock = 256;
+constexpr int kDefaultBlock = 256;   // cells per tile = threads per block
+constexpr int kMaxBlock = 256;
+#ifndef SWE_MIN_BLOCKS
+#define SWE_MIN_BLOCKS 3
+#endif
 constexpr int kMaxPart = 8192;       // upper bound on the grid of the step kernel
-__device__ __forceinline__ int chunk_count(int nt, int bs) { return (nt + bs - 1) / bs; }
+extern __shared__ __align__(32) unsigned char dyn_smem[];
 
 // One time step per launch.  Every block first reduces the per-block maxima of the previous
 // launch into dt (redundantly: a few KB from L2), so no separate finaliser launch and no atomics
-// sit between two steps; block 0 advances the device clock.
-__global__ void __launch_bounds__(kDefaultBlock)
+// sit between two steps; block 0 advances the device clock.  Blocks walk the tiles with a stride
+// of the grid.
+__global__ void __launch_bounds__(kMaxBlock, SWE_MIN_BLOCKS)
 swe_step_kernel(const Params P, const int cur)
 {
     __shared__ double s_red[32];
@@ -35,11 +40,8 @@ swe_step_kernel(const Params P, const int cur)
     Rec *__restrict__ Uout = P.U(cur ^ 1);
     double rate = 0.0;
     unsigned nclamp = 0;
-    const int nchunks = chunk_count(P.nt, blockDim.x);
-    for (int c = blockIdx.x; c < nchunks; c += gridDim.x) {
-        const int i = c * blockDim.x + threadIdx.x;
-        if (i < P.nt) rate = fmax(rate, update_cell<true>(P, Uin, Uout, i, dt, nclamp));
-    }
+    for (int t = blockIdx.x; t < P.ntiles; t += gridDim.x)
+        rate = fmax(rate, process_tile<true>(P, Uin, Uout, t, dt, nclamp, dyn_smem));
     rate = block_max(rate, s_red);
     if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
     if (threadIdx.x == 0) {
@@ -54,22 +56,19 @@ swe_step_kernel(const Params P, const int cur)
 
 // The whole time loop in one cooperative launch: grid barrier between steps instead of a kernel
 // boundary (small meshes are "strictly limited by latencies" of kernel launches).
-__global__ void __launch_bounds__(kDefaultBlock)
+__global__ void __launch_bounds__(kMaxBlock, SWE_MIN_BLOCKS)
 swe_persistent_kernel(const Params P, int cur, const long long nsteps)
 {
     __shared__ double s_red[32];
     cg::grid_group grid = cg::this_grid();
-    const int nchunks = chunk_count(P.nt, blockDim.x);
     for (long long s = 0; s < nsteps; s++) {
         const double dt = reduce_dt(P, P.pmax(cur), s_red);
         const Rec *Uin = P.U(cur);
         Rec *Uout = P.U(cur ^ 1);
         double rate = 0.0;
         unsigned nclamp = 0;
-        for (int c = blockIdx.x; c < nchunks; c += gridDim.x) {
-            const int i = c * blockDim.x + threadIdx.x;
-            if (i < P.nt) rate = fmax(rate, update_cell<false>(P, Uin, Uout, i, dt, nclamp));
-        }
+        for (int t = blockIdx.x; t < P.ntiles; t += gridDim.x)
+            rate = fmax(rate, process_tile<false>(P, Uin, Uout, t, dt, nclamp, dyn_smem));
         rate = block_max(rate, s_red);
         if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);
         if (threadIdx.x == 0) {
@@ -91,15 +90,12 @@ swe_rate_kernel(const Params P, const int cur)
 {
     __shared__ double s_red[32];
     double rate = 0.0;
-    const int nchunks = chunk_count(P.nt, blockDim.x);
-    for (int c = blockIdx.x; c < nchunks; c += gridDim.x) {
-        const int i = c * blockDim.x + threadIdx.x;
+    for (int t = blockIdx.x; t < P.ntiles; t += gridDim.x) {
+        const int i = t * blockDim.x + threadIdx.x;
         if (i < P.nt) {
             const Rec U = load_rec<true>(P.U(cur) + i);
-            if (U.h > P.hdry) {
-                const double2 cp = __ldg(P.cellp + i);
-                rate = fmax(rate, (sqrt(P.g * U.h) + sqrt(U.u * U.u + U.v * U.v)) * cp.x);
-            }
+            if (U.h > P.hdry)
+                rate = fmax(rate, (sqrt(P.g * U.h) + sqrt(U.u * U.u + U.v * U.v)) * P.cells[i].inv_R);
         }
     }
     rate = block_max(rate, s_red);
@@ -146,6 +142,7 @@ __global__ void swe_unpack_kernel(const Params P, const int cur, const int32_t *
 struct swe_mesh {
     swe_params prm;
     HostTables T;
+    TileTables X;
     std::string err;
     // device
     bool bound = false, have_state = false, have_rates = false;
@@ -155,6 +152,7 @@ struct swe_mesh {
     int32_t *d_perm = nullptr; double *d_zcell = nullptr; double *d_stage = nullptr;
     double *d_qn = nullptr;
     int cur = 0, grid = 0, block = kDefaultBlock, coop_grid = 0, loop_mode = SWE_LOOP_LAUNCH;
+    size_t smem = 0;          // dynamic shared memory of the step kernels
     int64_t launches = 0;
     double qn_tag[SWE_BC_MAX_TAG + 1] = {};
     std::map<std::pair<int, int>, cudaGraphExec_t> graphs; // (steps, cur) -> exec
@@ -174,16 +172,17 @@ static thread_local std::string g_create_err;
 static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 namespace {
+static_assert(sizeof(HostEdge) == sizeof(EdgeRec) && sizeof(HostCell) == sizeof(CellRec), "table records");
 struct Layout {
-    size_t U0, U1, nbr, nrm, coef, cellp, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
+    size_t U0, U1, cells, edges, estart, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
 };
-Layout make_layout(int64_t nt)
+Layout make_layout(const HostTables &T, const TileTables &X)
 {
-    Layout L; size_t o = 0; const size_t n = (size_t)nt;
+    Layout L; size_t o = 0; const size_t n = (size_t)T.nt;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     L.U0 = take(n * sizeof(Rec)); L.U1 = take(n * sizeof(Rec));
-    L.nbr = take(3 * n * sizeof(int32_t)); L.nrm = take(3 * n * sizeof(double2));
-    L.coef = take(3 * n * sizeof(double)); L.cellp = take(n * sizeof(double2));
+    L.cells = take(n * sizeof(CellRec)); L.edges = take(X.edges.size() * sizeof(EdgeRec));
+    L.estart = take(X.estart.size() * sizeof(int32_t));
     L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
     L.stage = take(3 * n * sizeof(double));
     L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
@@ -220,7 +219,7 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     if (params) p = *params;
     if (!(p.g > 0.0) || !(p.cfl > 0.0) || !(p.h_dry >= 0.0) || p.ordering < 0 || p.ordering > SWE_ORDER_RCM ||
         p.loop_mode < 0 || p.loop_mode > SWE_LOOP_LAUNCH ||
-        (p.block_size != 0 && (p.block_size < 64 || p.block_size > kDefaultBlock || p.block_size % 32))) {
+        (p.block_size != 0 && (p.block_size < 64 || p.block_size > kMaxBlock || p.block_size % 32))) {
         g_create_err = "swe_mesh_create: invalid swe_params (block_size must be a multiple of 32 in [64, 256])";
         return SWE_ERR_INVALID_ARG;
     }
@@ -233,6 +232,8 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     } catch (const std::bad_alloc &) { rc = SWE_ERR_NOMEM; m->err = "out of host memory"; }
     if (rc != SWE_OK) { g_create_err = m->err; delete m; return rc; }
     m->block = p.block_size ? p.block_size : kDefaultBlock;
+    rc = build_tiles(m->T, m->block, p.g, m->X, m->err);
+    if (rc != SWE_OK) { g_create_err = m->err; delete m; return rc; }
     *out = m;
     return SWE_OK;
 }
@@ -248,7 +249,7 @@ int swe_mesh_destroy(swe_mesh *m)
 int swe_mesh_workspace_bytes(const swe_mesh *m, size_t *bytes)
 {
     if (!m || !bytes) return SWE_ERR_INVALID_ARG;
-    *bytes = make_layout(m->T.nt).total;
+    *bytes = make_layout(m->T, m->X).total;
     return SWE_OK;
 }
 
@@ -288,7 +289,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     if (!m || !device_workspace) return SWE_ERR_INVALID_ARG;
     const HostTables &T = m->T;
     const size_t n = (size_t)T.nt;
-    const Layout L = make_layout(T.nt);
+    const Layout L = make_layout(T, m->X);
     if (bytes < L.total || ((uintptr_t)device_workspace & 255u)) {
         m->err = "workspace too small or not 256-byte aligned";
         return SWE_ERR_WORKSPACE;
@@ -297,59 +298,54 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     m->graphs.clear();
     m->bound = false; m->have_state = false; m->have_rates = false;
     m->ws = (char *)device_workspace; m->ws_bytes = bytes; m->stream = (cudaStream_t)cuda_stream;
-    int dev = 0, sms = 0, coop = 0;
+    int dev = 0, sms = 0, coop = 0, smem_optin = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+    CK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+    // dynamic shared memory: the tile's state records + five doubles per edge of the longest list
+    const TileTables &X = m->X;
+    m->smem = (size_t)m->block * sizeof(Rec) + (size_t)X.max_edges * 5 * sizeof(double);
+    if (m->smem > (size_t)smem_optin) { m->err = "tile does not fit in shared memory"; return SWE_ERR_CUDA; }
+    CK(cudaFuncSetAttribute(swe_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem));
+    CK(cudaFuncSetAttribute(swe_persistent_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem));
     int occ_step = 0, occ_pers = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_step, swe_step_kernel, m->block, 0));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_pers, swe_persistent_kernel, m->block, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_step, swe_step_kernel, m->block, m->smem));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_pers, swe_persistent_kernel, m->block, m->smem));
     if (occ_step < 1 || occ_pers < 1) { m->err = "kernel does not fit on this device"; return SWE_ERR_CUDA; }
-    const int nchunks = (int)((T.nt + m->block - 1) / m->block);
-    // grid: every SM holds its full complement of resident blocks, each walking chunks with a
-    // stride of the grid (a multiple of the SM count); small meshes get one block per chunk
-    m->grid = std::min(std::min(nchunks, sms * occ_step), kMaxPart);
-    m->coop_grid = std::min(std::min(nchunks, sms * occ_pers), kMaxPart);
+    const int ntiles = (int)X.ntiles;
+    // grid: every SM holds its full complement of resident blocks, each walking tiles with a
+    // stride of the grid (a multiple of the SM count); small meshes get one block per tile
+    m->grid = std::min(std::min(ntiles, sms * occ_step), kMaxPart);
+    m->coop_grid = std::min(std::min(ntiles, sms * occ_pers), kMaxPart);
     int mode = m->prm.loop_mode;
-    if (mode == SWE_LOOP_AUTO) mode = (coop && nchunks <= 2 * sms * occ_pers) ? SWE_LOOP_PERSISTENT : SWE_LOOP_GRAPH;
+    if (mode == SWE_LOOP_AUTO) mode = (coop && ntiles <= 2 * sms * occ_pers) ? SWE_LOOP_PERSISTENT : SWE_LOOP_GRAPH;
     if (mode == SWE_LOOP_PERSISTENT && !coop) mode = SWE_LOOP_GRAPH;
     m->loop_mode = mode;
 
     Params &P = m->P;
     P.U0 = (Rec *)(m->ws + L.U0); P.U1 = (Rec *)(m->ws + L.U1);
-    P.nbr = (const int32_t *)(m->ws + L.nbr); P.nrm = (const double2 *)(m->ws + L.nrm);
-    P.coef = (const double *)(m->ws + L.coef); P.cellp = (const double2 *)(m->ws + L.cellp);
+    P.cells = (const CellRec *)(m->ws + L.cells); P.edges = (const EdgeRec *)(m->ws + L.edges);
+    P.estart = (const int32_t *)(m->ws + L.estart);
     m->d_zcell = (double *)(m->ws + L.zcell); m->d_perm = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
     m->d_qn = (double *)(m->ws + L.qn); P.qn_tag = m->d_qn;
     P.ctrl = (Ctrl *)(m->ws + L.ctrl);
-    P.nt = (int32_t)T.nt;
+    P.nt = (int32_t)T.nt; P.ntiles = ntiles; P.max_edges = X.max_edges;
     P.npart = mode == SWE_LOOP_PERSISTENT ? m->coop_grid : m->grid;
-    P.g = m->prm.g; P.cfl = m->prm.cfl; P.hdry = m->prm.h_dry;
+    P.g = m->prm.g; P.inv_g = 1.0 / m->prm.g; P.cfl = m->prm.cfl;
+    // a side is dry iff h <= h_dry; the floor keeps every argument of the MUFU-seeded
+    // reciprocal / rsqrt a normal number when the caller asks for h_dry = 0
+    P.hdry = std::max(m->prm.h_dry, 1e-250);
 
-    // tables in the internal order, SoA over cells
     try {
-        std::vector<int32_t> nbr(3 * n);
-        std::vector<double> nrm(6 * n), coef(3 * n), cellp(2 * n), zc(n);
-        for (size_t p = 0; p < n; p++) {
-            const size_t c = (size_t)T.perm[p];
-            for (int k = 0; k < 3; k++) {
-                const int32_t j = T.nbr[3 * c + k];
-                nbr[(size_t)k * n + p] = j >= 0 ? T.inv[(size_t)j] : j;
-                nrm[2 * ((size_t)k * n + p)] = T.normal[6 * c + 2 * k];
-                nrm[2 * ((size_t)k * n + p) + 1] = T.normal[6 * c + 2 * k + 1];
-                coef[(size_t)k * n + p] = T.length[3 * c + k] / T.area[c];
-            }
-            cellp[2 * p] = 1.0 / T.inradius[c];
-            cellp[2 * p + 1] = m->prm.g * T.manning[c] * T.manning[c];
-            zc[p] = T.cell_z[c];
-        }
+        std::vector<double> zc(n);
+        for (size_t p = 0; p < n; p++) zc[p] = T.cell_z[(size_t)T.perm[p]];
         cudaStream_t s = m->stream;
-        CK(cudaMemcpyAsync(m->ws + L.nbr, nbr.data(), 3 * n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
-        CK(cudaMemcpyAsync(m->ws + L.nrm, nrm.data(), 6 * n * sizeof(double), cudaMemcpyHostToDevice, s));
-        CK(cudaMemcpyAsync(m->ws + L.coef, coef.data(), 3 * n * sizeof(double), cudaMemcpyHostToDevice, s));
-        CK(cudaMemcpyAsync(m->ws + L.cellp, cellp.data(), 2 * n * sizeof(double), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.cells, X.cells.data(), n * sizeof(CellRec), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.edges, X.edges.data(), X.edges.size() * sizeof(EdgeRec), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.estart, X.estart.data(), X.estart.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_zcell, zc.data(), n * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_perm, T.perm.data(), n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_qn, m->qn_tag, sizeof(m->qn_tag), cudaMemcpyHostToDevice, s));
@@ -458,7 +454,7 @@ int swe_compute_dt(swe_mesh *m, double *dt_out)
 static int launch_steps_direct(swe_mesh *m, int64_t n)
 {
     for (int64_t s = 0; s < n; s++) {
-        swe_step_kernel<<<m->grid, m->block, 0, m->stream>>>(m->P, m->cur);
+        swe_step_kernel<<<m->grid, m->block, m->smem, m->stream>>>(m->P, m->cur);
         m->cur ^= 1;
         m->launches++;
     }
@@ -478,7 +474,7 @@ static int graph_for(swe_mesh *m, int steps, cudaGraphExec_t *out)
     cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
     int c = m->cur;
     if (e == cudaSuccess) {
-        for (int s = 0; s < steps; s++) { swe_step_kernel<<<m->grid, m->block, 0, cap>>>(m->P, c); c ^= 1; }
+        for (int s = 0; s < steps; s++) { swe_step_kernel<<<m->grid, m->block, m->smem, cap>>>(m->P, c); c ^= 1; }
         e = cudaStreamEndCapture(cap, &g);
     }
     if (e == cudaSuccess) e = cudaGraphInstantiate(&ex, g, 0);
@@ -501,7 +497,7 @@ int swe_run(swe_mesh *m, int64_t nsteps)
     if (m->loop_mode == SWE_LOOP_PERSISTENT) {
         Params P = m->P; int cur = m->cur; long long ns = nsteps;
         void *args[] = { &P, &cur, &ns };
-        CK(cudaLaunchCooperativeKernel((void *)swe_persistent_kernel, dim3(m->coop_grid), dim3(m->block), args, 0, m->stream));
+        CK(cudaLaunchCooperativeKernel((void *)swe_persistent_kernel, dim3(m->coop_grid), dim3(m->block), args, m->smem, m->stream));
         m->launches++;
         m->cur ^= (int)(nsteps & 1);
         return SWE_OK;
