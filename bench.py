@@ -183,7 +183,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     loop = {"auto": B.LOOP_AUTO, "graph": B.LOOP_GRAPH, "persistent": B.LOOP_PERSISTENT,
             "launch": B.LOOP_LAUNCH}[args.loop]
     t_build = time.perf_counter()
-    m = B.SweMesh.from_workload(w, ordering=order, loop_mode=loop).bind_device(dev)
+    m = B.SweMesh.from_workload(w, ordering=order, loop_mode=loop, block_size=args.block).bind_device(dev)
     t_build = time.perf_counter() - t_build
     # pinned host buffers for the end-to-end leg
     pin = [torch.empty(n, dtype=torch.float64).pin_memory() for _ in range(6)]
@@ -281,6 +281,7 @@ def main():
     ap.add_argument("--workload", default="config4")
     ap.add_argument("--ordering", default="hilbert", choices=["hilbert", "rcm", "identity"])
     ap.add_argument("--loop", default="auto", choices=["auto", "graph", "persistent", "launch"])
+    ap.add_argument("--block", type=int, default=0, help="cells per tile = threads per block (0 = default)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)

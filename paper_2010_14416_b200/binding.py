@@ -56,7 +56,8 @@ def load_library(rebuild_if_stale: bool = True):
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.build() if rebuild_if_stale else _build.LIB
+    # SWE_B200_LIB: use a prebuilt library instead of (re)building the in-tree one
+    path = os.environ.get("SWE_B200_LIB") or (_build.build() if rebuild_if_stale else _build.LIB)
     L = C.CDLL(path)
     dp, i32p, i64 = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.c_int64
     vp = C.c_void_p

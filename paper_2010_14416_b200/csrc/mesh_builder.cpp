@@ -209,65 +209,55 @@ int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_
     return SWE_OK;
 }
 
-// ---- tile tables: each tile's unique edge list and each cell's three slots in it ---------------
+// ---- tile tables: each tile's unique edge list and its cells' constants -------------------------
 int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, std::string &err)
 {
     const int64_t nt = T.nt;
     const int TC = tile_cells;
-    if (TC < 32 || 3 * TC > 0x7fff) { err = "tile size out of range"; return SWE_ERR_INVALID_ARG; }
+    if (TC < 32 || TC > 1024) { err = "tile size out of range"; return SWE_ERR_INVALID_ARG; }
+    if (nt >= ((int64_t)1 << kHostIdBits)) { err = "more than 2^29 cells"; return SWE_ERR_INVALID_ARG; }
     try {
         X.tile_cells = TC;
         X.ntiles = (nt + TC - 1) / TC;
         X.estart.assign((size_t)X.ntiles + 1, 0);
-        X.cells.resize((size_t)nt);
+        X.cellc.assign((size_t)X.ntiles * 3 * TC, 1.0);
         X.edges.clear();
         X.edges.reserve((size_t)nt * 7 / 4 + 1024);
         X.max_edges = 0;
-        std::vector<uint16_t> slot((size_t)TC * 3);
         auto local_edge_towards = [&](int32_t c, int32_t other) {   // k with nbr(c,k) == other
             for (int k = 0; k < 3; k++) if (T.nbr[3 * (size_t)c + k] == other) return k;
             return -1;
         };
+        auto enc = [](int64_t p, int k) { return (int32_t)(p | ((int64_t)k << kHostIdBits)); };
         for (int64_t t = 0; t < X.ntiles; t++) {
             const int64_t base = t * TC, nc = std::min<int64_t>(TC, nt - base);
             const size_t first = X.edges.size();
+            double *cc = X.cellc.data() + (size_t)t * 3 * TC;
+            for (int64_t q = 0; q < TC; q++) cc[2 * TC + q] = 0.0;
             for (int64_t q = 0; q < nc; q++) {
                 const int64_t p = base + q;
                 const int32_t c = T.perm[(size_t)p];
                 for (int k = 0; k < 3; k++) {
                     const int32_t j = T.nbr[3 * (size_t)c + k];
-                    uint16_t s;
+                    const double *nk = &T.normal[6 * (size_t)c + 2 * k];
                     if (j < 0) {                                   // boundary edge: a = this cell
-                        s = (uint16_t)(X.edges.size() - first);
-                        X.edges.push_back({ (int32_t)p, j, T.normal[6 * (size_t)c + 2 * k],
-                                            T.normal[6 * (size_t)c + 2 * k + 1], T.length[3 * (size_t)c + k] });
-                    } else {
-                        const int64_t pj = T.inv[(size_t)j];
-                        const int kj = local_edge_towards(j, c);
-                        if (kj < 0) { err = "inconsistent neighbour table"; return SWE_ERR_NON_MANIFOLD; }
-                        const bool in_tile = pj >= base && pj < base + nc;
-                        const bool am_b = j < c;                   // a = smaller caller id (R-17)
-                        if (in_tile && pj < p) {                   // emitted when pj was visited
-                            s = (uint16_t)(slot[(size_t)(pj - base) * 3 + kj] & 0x7fffu);
-                        } else {
-                            s = (uint16_t)(X.edges.size() - first);
-                            if (!am_b)
-                                X.edges.push_back({ (int32_t)p, (int32_t)pj, T.normal[6 * (size_t)c + 2 * k],
-                                                    T.normal[6 * (size_t)c + 2 * k + 1], T.length[3 * (size_t)c + k] });
-                            else
-                                X.edges.push_back({ (int32_t)pj, (int32_t)p, T.normal[6 * (size_t)j + 2 * kj],
-                                                    T.normal[6 * (size_t)j + 2 * kj + 1], T.length[3 * (size_t)j + kj] });
-                        }
-                        if (am_b) s |= 0x8000u;
+                        X.edges.push_back({ enc(p, k), j, nk[0], nk[1], T.length[3 * (size_t)c + k] });
+                        continue;
                     }
-                    slot[(size_t)q * 3 + k] = s;
+                    const int64_t pj = T.inv[(size_t)j];
+                    const bool in_tile = pj >= base && pj < base + nc;
+                    if (in_tile && pj < p) continue;               // emitted when pj was visited
+                    const int kj = local_edge_towards(j, c);
+                    if (kj < 0) { err = "inconsistent neighbour table"; return SWE_ERR_NON_MANIFOLD; }
+                    if (c < j)                                     // a = smaller caller id (R-17)
+                        X.edges.push_back({ enc(p, k), enc(pj, kj), nk[0], nk[1], T.length[3 * (size_t)c + k] });
+                    else
+                        X.edges.push_back({ enc(pj, kj), enc(p, k), T.normal[6 * (size_t)j + 2 * kj],
+                                            T.normal[6 * (size_t)j + 2 * kj + 1], T.length[3 * (size_t)j + kj] });
                 }
-                HostCell &hc = X.cells[(size_t)p];
-                hc.slots01 = (uint32_t)slot[(size_t)q * 3] | ((uint32_t)slot[(size_t)q * 3 + 1] << 16);
-                hc.slots2 = slot[(size_t)q * 3 + 2];
-                hc.inv_area = 1.0 / T.area[(size_t)c];
-                hc.inv_R = 1.0 / T.inradius[(size_t)c];
-                hc.gm2 = g * T.manning[(size_t)c] * T.manning[(size_t)c];
+                cc[q] = 1.0 / T.area[(size_t)c];
+                cc[TC + q] = 1.0 / T.inradius[(size_t)c];
+                cc[2 * TC + q] = g * T.manning[(size_t)c] * T.manning[(size_t)c];
             }
             const size_t cnt = X.edges.size() - first;
             if (X.edges.size() > (size_t)INT32_MAX) { err = "too many edges"; return SWE_ERR_INVALID_ARG; }

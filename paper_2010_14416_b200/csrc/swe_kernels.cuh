@@ -1,16 +1,18 @@
 // Device code of libswe_b200: the fused, tiled, edge-once SWE step for sm_100a (FP64).
 //
 // The cells are numbered along a space-filling curve (mesh_builder.cpp) and cut into tiles of
-// blockDim.x consecutive cells.  One thread block processes one tile at a time:
+// blockDim.x consecutive cells.  A thread block walks tiles through a two-stage pipeline:
 //
-//   phase 0  every thread loads its own cell's state record (one 256-bit load) into shared
-//            memory and registers, its cell-table record, and the first edge record it will
-//            evaluate; edge end points that live in another tile are gathered from global
-//            memory right away so that their latency overlaps the barrier
+//   stage    one elected thread issues three TMA bulk copies (cp.async.bulk, mbarrier
+//            complete_tx) for the tile's three CONTIGUOUS streams: the state records of its
+//            cells, its edge list and its cell constants.  The copies for tile n+1 are in
+//            flight while tile n is computed; nothing passes through registers.
 //   phase 1  (edge-parallel) every edge that touches the tile is evaluated ONCE: hydrostatic
 //            reconstruction, rotation, HLLC flux, rotation back, both sides' bathymetry source;
-//            five doubles per edge go to shared memory (a1-a7 of SURVEY.md section 8(a))
-//   phase 2  (cell-parallel) every cell sums its three edges in the fixed order k = 0,1,2,
+//            the signed, length-weighted result goes to the (cell, local edge) slots of its end
+//            points in shared memory (a1-a7 of SURVEY.md section 8(a)).  End points in another
+//            tile are the only gathers from global memory (one 32-byte sector each).
+//   phase 2  (cell-parallel) every cell sums its three slots in the fixed order k = 0,1,2,
 //            applies the semi-implicit friction and the update, writes its new record with
 //            one 256-bit store and contributes (sqrt(g h)+|V|)/R of the NEW state to the block
 //            maximum (a7-a11)
@@ -24,9 +26,9 @@
 //
 // Arithmetic: FP64 throughout.  Division and square root are the FP64 pipe's dominant cost on
 // wet meshes (profiles/r01_v1_README.md), so the kernels use the MUFU seeds (rcp/rsqrt.approx)
-// with a third-order correction (error ~1 ulp, no special-case handling: every argument is a
-// normal positive number by construction) instead of the IEEE-rounded sequences.
-// section 7 derives why this stays inside the 1e-10 parity bar.
+// with a third-order correction (measured max error 1.1-1.5e-16, no special-case handling:
+// every argument is a normal positive number by construction) instead of the IEEE-rounded
+// sequences.  DESIGN.md section 7 derives why this stays inside the 1e-10 parity bar.
 #pragma once
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
@@ -39,11 +41,11 @@ struct __align__(32) Rec { double h, u, v, z; };
 // One edge of a tile.  a is always a cell; b is a cell or -tag on a boundary edge.  (n1,n2) is
 // a's unit outward normal on this edge (so b's is its negative).  a is the end point with the
 // smaller CALLER id, which makes the result independent of the renumbering (R-17).
+// Cell ids are internal ids in bits 0-28; bits 29-30 hold the local edge index k of this edge
+// in that cell.
 struct __align__(32) EdgeRec { int32_t a, b; double n1, n2, len; };
-
-// Per-cell constants.  slot k (16 bits): bits 0-14 = index of local edge k in the tile's edge
-// list, bit 15 = 1 if this cell is the edge's b side.
-struct __align__(32) CellRec { uint32_t slots01, slots2; double inv_area, inv_R, gm2; };
+constexpr int kIdBits = 29;
+constexpr int32_t kIdMask = (1 << kIdBits) - 1;
 
 struct Ctrl {                 // device-resident loop state
     double t;                 // simulated time
@@ -57,7 +59,7 @@ struct Ctrl {                 // device-resident loop state
 
 struct Params {
     Rec *U0, *U1;             // ping-pong state, internal order
-    const CellRec *cells;     // [nt]
+    const double *cellc;      // [ntiles][3][tile] per tile: 1/|Omega|, 1/R, g m^2 (SoA, padded)
     const EdgeRec *edges;     // [estart[ntiles]] tile after tile
     const int32_t *estart;    // [ntiles + 1]
     const double *qn_tag;     // [128] unit discharge along the outward normal per inflow tag
@@ -71,16 +73,14 @@ struct Params {
 };
 
 // ---- 256-bit access --------------------------------------------------------------------------
-template <bool kReadOnlyPath>
+// Gather of a record of another tile: L2-coherent (.cg), because in the persistent loop other
+// blocks rewrote the state before the grid barrier; L1 would add nothing (each such record is
+// used about once per tile).
 __device__ __forceinline__ Rec load_rec(const Rec *p)
 {
     Rec r;
-    if (kReadOnlyPath)   // state is constant for the whole launch
-        asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
-                     : "=d"(r.h), "=d"(r.u), "=d"(r.v), "=d"(r.z) : "l"(p));
-    else                 // persistent loop: other blocks rewrote it before the grid barrier
-        asm volatile("ld.global.cg.v4.f64 {%0,%1,%2,%3}, [%4];"
-                     : "=d"(r.h), "=d"(r.u), "=d"(r.v), "=d"(r.z) : "l"(p) : "memory");
+    asm volatile("ld.global.cg.v4.f64 {%0,%1,%2,%3}, [%4];"
+                 : "=d"(r.h), "=d"(r.u), "=d"(r.v), "=d"(r.z) : "l"(p) : "memory");
     return r;
 }
 __device__ __forceinline__ void store_rec(Rec *p, const Rec &r)
@@ -88,29 +88,11 @@ __device__ __forceinline__ void store_rec(Rec *p, const Rec &r)
     asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};"
                  :: "l"(p), "d"(r.h), "d"(r.u), "d"(r.v), "d"(r.z) : "memory");
 }
-__device__ __forceinline__ EdgeRec load_edge(const EdgeRec *p)
-{
-    EdgeRec e; double ab;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
-                 : "=d"(ab), "=d"(e.n1), "=d"(e.n2), "=d"(e.len) : "l"(p));
-    const long long w = __double_as_longlong(ab);
-    e.a = (int32_t)(w & 0xffffffffll); e.b = (int32_t)(w >> 32);
-    return e;
-}
-__device__ __forceinline__ CellRec load_cell(const CellRec *p)
-{
-    CellRec c; double s;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0,%1,%2,%3}, [%4];"
-                 : "=d"(s), "=d"(c.inv_area), "=d"(c.inv_R), "=d"(c.gm2) : "l"(p));
-    const long long w = __double_as_longlong(s);
-    c.slots01 = (uint32_t)(w & 0xffffffffll); c.slots2 = (uint32_t)((unsigned long long)w >> 32);
-    return c;
-}
-
 // ---- MUFU-seeded FP64 reciprocal / rsqrt / rcbrt ---------------------------------------------
 // Arguments are finite, normal and positive at every call site (depths above the wet/dry
 // threshold, sums of celerities, S_R - S_L in the star region, determinants >= 1).
-// Seed relative error e0 <= ~2^-20; the corrections below leave O(e0^3) + rounding (~1 ulp).
+// Seed relative error e0 <= ~2^-20; the corrections below leave O(e0^3) + rounding: measured
+// max relative error 1.1e-16 (rcp), 1.4e-16 (rsqrt), 1.5e-16 (rcbrt) over 2^-60..2^60.
 __device__ __forceinline__ double fast_rcp(double x)
 {
     double y;
@@ -272,37 +254,27 @@ __device__ __forceinline__ void edge_eval(const Params &P, const EdgeRec &er, co
 }
 
 // ---- one cell: a7-a10, eq.(37), PAPER.md:250 ---------------------------------------------------
-// so = the tile's edge outputs in shared memory (SoA, stride ME).  Returns the local rate
-// (sqrt(g h') + |V'|) / R_i of the new state (0 if dry), eq.(15).
-__device__ __forceinline__ double cell_update(const Params &P, const Rec &Ui, const CellRec &ct,
-                                              const double *so, const int ME, const double dt,
-                                              Rec &Un, unsigned &nclamp)
+// (s1,s2,s3) = sum over the three edges of the signed, length-weighted flux + source.  Returns
+// the local rate (sqrt(g h') + |V'|) / R_i of the new state (0 if dry), eq.(15).
+__device__ __forceinline__ double cell_update(const Params &P, const Rec &Ui, const double s1,
+                                              const double s2, const double s3,
+                                              const double inv_area, const double inv_R,
+                                              const double gm2, const double dt, Rec &Un,
+                                              unsigned &nclamp)
 {
     const double g = P.g, hdry = P.hdry;
     const double hi = Ui.h, ui = Ui.u, vi = Ui.v;
-    // three edges in the fixed order k = 0,1,2 (R-17)
-    double s1 = 0.0, s2 = 0.0, s3 = 0.0;
-#pragma unroll
-    for (int k = 0; k < 3; k++) {
-        const uint32_t w = k == 0 ? ct.slots01 : k == 1 ? ct.slots01 >> 16 : ct.slots2;
-        const int e = (int)(w & 0x7fffu);
-        const bool bside = (w & 0x8000u) != 0;
-        const double *q = so + e;
-        const double o0 = q[0];
-        const double ox = q[(bside ? 3 : 1) * ME], oy = q[(bside ? 4 : 2) * ME];
-        if (bside) { s1 -= o0; s2 -= ox; s3 -= oy; } else { s1 += o0; s2 += ox; s3 += oy; }
-    }
-    const double b1 = -ct.inv_area * s1, b2 = -ct.inv_area * s2, b3 = -ct.inv_area * s3;
+    const double b1 = -inv_area * s1, b2 = -inv_area * s2, b3 = -inv_area * s3;
     // a8: semi-implicit friction, eq.(32)-(37), R-19
     const double qx = hi * ui, qy = hi * vi;
     const double dh = dt * b1;
     double r2 = dt * b2, r3 = dt * b3, dqx, dqy;
     const double qq2 = qx * qx + qy * qy;
-    if (hi > hdry && ct.gm2 > 0.0 && qq2 > 1e-200) {
+    if (hi > hdry && gm2 > 0.0 && qq2 > 1e-200) {
         const double rq = fast_rsqrt(qq2), qq = qq2 * rq;
         const double c3 = (hi > 1e-28 && hi < 1e28) ? fast_rcbrt(hi) : rcbrt(hi);   // h^(-1/3)
         const double c32 = c3 * c3, rh = c32 * c3;              // h^(-2/3), 1/h
-        const double cfr = ct.gm2 * (rh * rh) * c3;             // g m^2 / h^(7/3)
+        const double cfr = gm2 * (rh * rh) * c3;                // g m^2 / h^(7/3)
         const double S2 = -cfr * qx * qq, S3 = -cfr * qy * qq;
         const double k73 = (7.0 / 3.0) * cfr * qq * rh;
         const double J21 = k73 * qx, J31 = k73 * qy;
@@ -329,68 +301,157 @@ __device__ __forceinline__ double cell_update(const Params &P, const Rec &Ui, co
         const double ghn = g * hn, a = ghn * fast_rsqrt(ghn);
         const double v2 = Un.u * Un.u + Un.v * Un.v;
         const double vm = v2 > 1e-200 ? v2 * fast_rsqrt(v2) : 0.0;
-        rate = (a + vm) * ct.inv_R;
+        rate = (a + vm) * inv_R;
     } else { Un.u = 0.0; Un.v = 0.0; }
     return rate;
 }
 
-// ---- one tile ------------------------------------------------------------------------------------
-// smem: Rec srec[blockDim.x] followed by double so[5][ME].  Two block barriers per tile; the
-// caller needs none between tiles (srec is read only before the second barrier, so is written
-// only after the next tile's first barrier).
-template <bool kReadOnlyPath>
-__device__ __forceinline__ double process_tile(const Params &P, const Rec *__restrict__ Uin,
-                                               Rec *__restrict__ Uout, const int tile,
-                                               const double dt, unsigned &nclamp,
-                                               unsigned char *smem)
+// ---- TMA bulk copy + mbarrier (sm_90+/sm_100a) ---------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
 {
-    const int TC = blockDim.x, tid = threadIdx.x, ME = P.max_edges;
-    const int base = tile * TC, i = base + tid;
-    const bool active = i < P.nt;
-    Rec *srec = reinterpret_cast<Rec *>(smem);
-    double *so = reinterpret_cast<double *>(smem + (size_t)TC * sizeof(Rec));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+                 "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+                 :: "r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// bytes: multiple of 16; src and dst 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// ---- the tile pipeline -----------------------------------------------------------------------------
+// Shared memory of one block (dynamic), TC = blockDim.x, ME = P.max_edges:
+//   double  so[9][TC]            (k, component) slots of the tile's cells
+//   per stage s = 0..kStages-1:  Rec srec[TC]; double scell[3][TC]; EdgeRec sedge[ME]
+//   uint64  bar[kStages]
+#ifndef SWE_STAGES
+#define SWE_STAGES 2
+#endif
+constexpr int kStages = SWE_STAGES;   // 2: the next tile's copies fly during this tile's compute
+__host__ __device__ __forceinline__ size_t stage_bytes(int TC, int ME)
+{
+    return (size_t)TC * sizeof(Rec) + (size_t)TC * 3 * sizeof(double) + (size_t)ME * sizeof(EdgeRec);
+}
+__host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int ME)
+{
+    return (size_t)TC * 9 * sizeof(double) + kStages * stage_bytes(TC, ME) + kStages * sizeof(uint64_t);
+}
+
+struct TilePipe {
+    double *so; unsigned char *stage0; uint64_t *bar; size_t sbytes;
+    __device__ __forceinline__ Rec *srec(int s) const { return reinterpret_cast<Rec *>(stage0 + s * sbytes); }
+    __device__ __forceinline__ double *scell(int s, int TC) const
+    { return reinterpret_cast<double *>(stage0 + s * sbytes + (size_t)TC * sizeof(Rec)); }
+    __device__ __forceinline__ EdgeRec *sedge(int s, int TC) const
+    { return reinterpret_cast<EdgeRec *>(stage0 + s * sbytes + (size_t)TC * (sizeof(Rec) + 3 * sizeof(double))); }
+};
+__device__ __forceinline__ TilePipe make_pipe(const Params &P, unsigned char *smem)
+{
+    const int TC = blockDim.x;
+    TilePipe p;
+    p.so = reinterpret_cast<double *>(smem);
+    p.stage0 = smem + (size_t)TC * 9 * sizeof(double);
+    p.sbytes = stage_bytes(TC, P.max_edges);
+    p.bar = reinterpret_cast<uint64_t *>(p.stage0 + kStages * p.sbytes);
+    return p;
+}
+// one thread: arm the stage's barrier and start the three bulk copies of `tile`
+__device__ __forceinline__ void issue_tile(const Params &P, const TilePipe &pp, const Rec *Uin,
+                                           const int tile, const int s)
+{
+    const int TC = blockDim.x;
+    const int base = tile * TC, nc = min(TC, P.nt - base);
     const int e0 = __ldg(P.estart + tile), ne = __ldg(P.estart + tile + 1) - e0;
-    // ---- phase 0
-    Rec Ui; CellRec ct;
-    if (active) {
-        Ui = load_rec<kReadOnlyPath>(Uin + i);
-        ct = load_cell(P.cells + i);
-    }
-    EdgeRec er; Rec A, B;
-    bool offA = false, offB = false;
-    if (tid < ne) {
-        er = load_edge(P.edges + e0 + tid);
-        offA = (unsigned)(er.a - base) >= (unsigned)TC;
-        offB = er.b >= 0 && (unsigned)(er.b - base) >= (unsigned)TC;
-        if (offA) A = load_rec<kReadOnlyPath>(Uin + er.a);
-        if (offB) B = load_rec<kReadOnlyPath>(Uin + er.b);
-    }
-    if (active) srec[tid] = Ui;
-    __syncthreads();
-    // ---- phase 1: every edge of the tile once
-    for (int e = tid; e < ne; e += TC) {
-        if (e != tid) {
-            er = load_edge(P.edges + e0 + e);
-            offA = (unsigned)(er.a - base) >= (unsigned)TC;
-            offB = er.b >= 0 && (unsigned)(er.b - base) >= (unsigned)TC;
-            if (offA) A = load_rec<kReadOnlyPath>(Uin + er.a);
-            if (offB) B = load_rec<kReadOnlyPath>(Uin + er.b);
-        }
-        if (!offA) A = srec[er.a - base];
-        if (er.b >= 0 && !offB) B = srec[er.b - base];
-        double o[5];
-        edge_eval(P, er, A, B, o);
-#pragma unroll
-        for (int c = 0; c < 5; c++) so[c * ME + e] = o[c];
-    }
-    __syncthreads();
-    // ---- phase 2: every cell of the tile
+    const unsigned b_rec = (unsigned)nc * sizeof(Rec), b_cell = (unsigned)TC * 3 * sizeof(double),
+                   b_edge = (unsigned)ne * sizeof(EdgeRec);
+    mbar_expect_tx(pp.bar + s, b_rec + b_cell + b_edge);
+    bulk_g2s(pp.srec(s), Uin + base, b_rec, pp.bar + s);
+    bulk_g2s(pp.scell(s, TC), P.cellc + (size_t)tile * 3 * TC, b_cell, pp.bar + s);
+    bulk_g2s(pp.sedge(s, TC), P.edges + e0, b_edge, pp.bar + s);
+}
+
+// All the tiles of this block for one time step.  `it0` = number of tiles this block has pushed
+// through the pipeline before (persistent loop), which fixes stage and barrier parity.
+// Returns the block-local maximum rate contribution of this thread.
+__device__ __forceinline__ double step_tiles(const Params &P, const TilePipe &pp,
+                                             const Rec *__restrict__ Uin, Rec *__restrict__ Uout,
+                                             const double dt, unsigned &nclamp, unsigned &it0)
+{
+    const int TC = blockDim.x, tid = threadIdx.x;
     double rate = 0.0;
-    if (active) {
-        Rec Un;
-        rate = cell_update(P, Ui, ct, so, ME, dt, Un, nclamp);
-        store_rec(Uout + i, Un);
+    unsigned it = it0;
+    int tile = blockIdx.x;
+    if (tile >= P.ntiles) return 0.0;
+    if (kStages > 1 && tid == 0) issue_tile(P, pp, Uin, tile, it % kStages);
+    for (; tile < P.ntiles; tile += gridDim.x, it++) {
+        const int s = it % kStages;
+        const int base = tile * TC;
+        const int ne = __ldg(P.estart + tile + 1) - __ldg(P.estart + tile);
+        if (kStages > 1) {
+            mbar_wait(pp.bar + s, (it / kStages) & 1u);
+            __syncthreads();      // every thread has left the previous tile: so[] and the other stage are free
+            if (tid == 0 && tile + (int)gridDim.x < P.ntiles)
+                issue_tile(P, pp, Uin, tile + gridDim.x, (it + 1) % kStages);
+        } else {
+            __syncthreads();
+            if (tid == 0) issue_tile(P, pp, Uin, tile, 0);
+            mbar_wait(pp.bar, it & 1u);
+        }
+        const Rec *srec = pp.srec(s);
+        const EdgeRec *sedge = pp.sedge(s, TC);
+        double *so = pp.so;
+        // ---- phase 1: every edge of the tile once
+        for (int e = tid; e < ne; e += TC) {
+            const EdgeRec er = sedge[e];
+            const int ia = (er.a & kIdMask) - base, ka = er.a >> kIdBits;
+            const bool inA = (unsigned)ia < (unsigned)TC;
+            Rec A, B;
+            if (inA) A = srec[ia]; else A = load_rec(Uin + (er.a & kIdMask));
+            int ib = -1, kb = 0; bool inB = false;
+            if (er.b >= 0) {
+                ib = (er.b & kIdMask) - base; kb = er.b >> kIdBits;
+                inB = (unsigned)ib < (unsigned)TC;
+                if (inB) B = srec[ib]; else B = load_rec(Uin + (er.b & kIdMask));
+            }
+            double o[5];
+            edge_eval(P, er, A, B, o);
+            if (inA) {
+                double *q = so + (ka * 3) * TC + ia;
+                q[0] = o[0]; q[TC] = o[1]; q[2 * TC] = o[2];
+            }
+            if (inB) {
+                double *q = so + (kb * 3) * TC + ib;
+                q[0] = -o[0]; q[TC] = -o[3]; q[2 * TC] = -o[4];
+            }
+        }
+        __syncthreads();
+        // ---- phase 2: every cell of the tile
+        const int i = base + tid;
+        if (i < P.nt) {
+            const Rec Ui = srec[tid];
+            const double *sc = pp.scell(s, TC) + tid;
+            const double *q = so + tid;
+            // three edges in the fixed order k = 0,1,2 (R-17)
+            const double s1 = (q[0] + q[3 * TC]) + q[6 * TC];
+            const double s2 = (q[TC] + q[4 * TC]) + q[7 * TC];
+            const double s3 = (q[2 * TC] + q[5 * TC]) + q[8 * TC];
+            Rec Un;
+            rate = fmax(rate, cell_update(P, Ui, s1, s2, s3, sc[0], sc[TC], sc[2 * TC], dt, Un, nclamp));
+            store_rec(Uout + i, Un);
+        }
     }
+    it0 = it;
     return rate;
 }
 

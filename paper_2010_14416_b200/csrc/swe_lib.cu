@@ -27,50 +27,37 @@ constexpr int kMaxBlock = 256;
 constexpr int kMaxPart = 8192;       // upper bound on the grid of the step kernel
 extern __shared__ __align__(32) unsigned char dyn_smem[];
 
-// One time step per launch.  Every block first reduces the per-block maxima of the previous
-// launch into dt (redundantly: a few KB from L2), so no separate finaliser launch and no atomics
-// sit between two steps; block 0 advances the device clock.  Blocks walk the tiles with a stride
-// of the grid.
-__global__ void __launch_bounds__(kMaxBlock, SWE_MIN_BLOCKS)
-swe_step_kernel(const Params P, const int cur)
+__device__ __forceinline__ TilePipe pipe_setup(const Params &P)
 {
-    __shared__ double s_red[32];
-    const double dt = reduce_dt(P, P.pmax(cur), s_red);
-    const Rec *__restrict__ Uin = P.U(cur);
-    Rec *__restrict__ Uout = P.U(cur ^ 1);
-    double rate = 0.0;
-    unsigned nclamp = 0;
-    for (int t = blockIdx.x; t < P.ntiles; t += gridDim.x)
-        rate = fmax(rate, process_tile<true>(P, Uin, Uout, t, dt, nclamp, dyn_smem));
-    rate = block_max(rate, s_red);
-    if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
+    const TilePipe pp = make_pipe(P, dyn_smem);
     if (threadIdx.x == 0) {
-        P.pmax(cur ^ 1)[blockIdx.x] = rate;
-        if (blockIdx.x == 0) {
-            Ctrl *c = P.ctrl;
-            c->t += dt; c->dt_last = dt; c->steps += 1;
-            if (!(dt > 0.0)) c->all_dry = 1;
-        }
+        for (int s = 0; s < kStages; s++) mbar_init(pp.bar + s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    __syncthreads();
+    return pp;
 }
 
-// The whole time loop in one cooperative launch: grid barrier between steps instead of a kernel
-// boundary (small meshes are "strictly limited by latencies" of kernel launches).
+// nsteps time steps.  Every block first reduces the per-block maxima of the previous step into
+// dt (redundantly: a few KB from L2), so no separate finaliser launch and no atomics sit between
+// two steps; block 0 advances the device clock.  Blocks walk the tiles with a stride of the grid
+// through the two-stage TMA pipeline of swe_kernels.cuh.
+//   graph / launch mode: nsteps = 1 per launch, the kernel boundary separates the steps;
+//   persistent mode: one cooperative launch runs the whole loop with a grid barrier between
+//   steps (small meshes are "strictly limited by latencies" of kernel launches).
+// One kernel serves all modes, so their results are bitwise identical by construction.
 __global__ void __launch_bounds__(kMaxBlock, SWE_MIN_BLOCKS)
-swe_persistent_kernel(const Params P, int cur, const long long nsteps)
+swe_step_kernel(const Params P, int cur, const long long nsteps)
 {
     __shared__ double s_red[32];
-    cg::grid_group grid = cg::this_grid();
+    const TilePipe pp = pipe_setup(P);
+    unsigned it = 0;
     for (long long s = 0; s < nsteps; s++) {
         const double dt = reduce_dt(P, P.pmax(cur), s_red);
-        const Rec *Uin = P.U(cur);
-        Rec *Uout = P.U(cur ^ 1);
-        double rate = 0.0;
         unsigned nclamp = 0;
-        for (int t = blockIdx.x; t < P.ntiles; t += gridDim.x)
-            rate = fmax(rate, process_tile<false>(P, Uin, Uout, t, dt, nclamp, dyn_smem));
+        double rate = step_tiles(P, pp, P.U(cur), P.U(cur ^ 1), dt, nclamp, it);
         rate = block_max(rate, s_red);
-        if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);
+        if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
         if (threadIdx.x == 0) {
             P.pmax(cur ^ 1)[blockIdx.x] = rate;
             if (blockIdx.x == 0) {
@@ -80,7 +67,11 @@ swe_persistent_kernel(const Params P, int cur, const long long nsteps)
             }
         }
         cur ^= 1;
-        grid.sync();
+        if (s + 1 < nsteps) {     // only reached in a cooperative launch
+            // the next step's bulk copies (async proxy) read what this step's threads stored
+            asm volatile("fence.proxy.async;" ::: "memory");
+            cg::this_grid().sync();
+        }
     }
 }
 
@@ -93,9 +84,10 @@ swe_rate_kernel(const Params P, const int cur)
     for (int t = blockIdx.x; t < P.ntiles; t += gridDim.x) {
         const int i = t * blockDim.x + threadIdx.x;
         if (i < P.nt) {
-            const Rec U = load_rec<true>(P.U(cur) + i);
+            const Rec U = load_rec(P.U(cur) + i);
             if (U.h > P.hdry)
-                rate = fmax(rate, (sqrt(P.g * U.h) + sqrt(U.u * U.u + U.v * U.v)) * P.cells[i].inv_R);
+                rate = fmax(rate, (sqrt(P.g * U.h) + sqrt(U.u * U.u + U.v * U.v)) *
+                                  __ldg(P.cellc + ((size_t)t * 3 + 1) * blockDim.x + threadIdx.x));
         }
     }
     rate = block_max(rate, s_red);
@@ -128,7 +120,7 @@ __global__ void swe_unpack_kernel(const Params P, const int cur, const int32_t *
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P.nt) return;
     const int c = perm[p];
-    const Rec r = load_rec<true>(P.U(cur) + p);
+    const Rec r = load_rec(P.U(cur) + p);
     if (h) h[c] = r.h;
     if (hu) hu[c] = r.h * r.u;
     if (hv) hv[c] = r.h * r.v;
@@ -172,16 +164,16 @@ static thread_local std::string g_create_err;
 static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 namespace {
-static_assert(sizeof(HostEdge) == sizeof(EdgeRec) && sizeof(HostCell) == sizeof(CellRec), "table records");
+static_assert(sizeof(HostEdge) == sizeof(EdgeRec) && kHostIdBits == kIdBits, "table records");
 struct Layout {
-    size_t U0, U1, cells, edges, estart, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
+    size_t U0, U1, cellc, edges, estart, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
 };
 Layout make_layout(const HostTables &T, const TileTables &X)
 {
     Layout L; size_t o = 0; const size_t n = (size_t)T.nt;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     L.U0 = take(n * sizeof(Rec)); L.U1 = take(n * sizeof(Rec));
-    L.cells = take(n * sizeof(CellRec)); L.edges = take(X.edges.size() * sizeof(EdgeRec));
+    L.cellc = take(X.cellc.size() * sizeof(double)); L.edges = take(X.edges.size() * sizeof(EdgeRec));
     L.estart = take(X.estart.size() * sizeof(int32_t));
     L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
     L.stage = take(3 * n * sizeof(double));
@@ -303,15 +295,14 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     CK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-    // dynamic shared memory: the tile's state records + five doubles per edge of the longest list
+    // dynamic shared memory: flux slots + two stages of {state records, cell constants, longest edge list}
     const TileTables &X = m->X;
-    m->smem = (size_t)m->block * sizeof(Rec) + (size_t)X.max_edges * 5 * sizeof(double);
+    m->smem = tile_smem_bytes(m->block, X.max_edges);
     if (m->smem > (size_t)smem_optin) { m->err = "tile does not fit in shared memory"; return SWE_ERR_CUDA; }
     CK(cudaFuncSetAttribute(swe_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem));
-    CK(cudaFuncSetAttribute(swe_persistent_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem));
     int occ_step = 0, occ_pers = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_step, swe_step_kernel, m->block, m->smem));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_pers, swe_persistent_kernel, m->block, m->smem));
+    occ_pers = occ_step;
     if (occ_step < 1 || occ_pers < 1) { m->err = "kernel does not fit on this device"; return SWE_ERR_CUDA; }
     const int ntiles = (int)X.ntiles;
     // grid: every SM holds its full complement of resident blocks, each walking tiles with a
@@ -325,7 +316,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
 
     Params &P = m->P;
     P.U0 = (Rec *)(m->ws + L.U0); P.U1 = (Rec *)(m->ws + L.U1);
-    P.cells = (const CellRec *)(m->ws + L.cells); P.edges = (const EdgeRec *)(m->ws + L.edges);
+    P.cellc = (const double *)(m->ws + L.cellc); P.edges = (const EdgeRec *)(m->ws + L.edges);
     P.estart = (const int32_t *)(m->ws + L.estart);
     m->d_zcell = (double *)(m->ws + L.zcell); m->d_perm = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
@@ -343,7 +334,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
         std::vector<double> zc(n);
         for (size_t p = 0; p < n; p++) zc[p] = T.cell_z[(size_t)T.perm[p]];
         cudaStream_t s = m->stream;
-        CK(cudaMemcpyAsync(m->ws + L.cells, X.cells.data(), n * sizeof(CellRec), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.cellc, X.cellc.data(), X.cellc.size() * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.edges, X.edges.data(), X.edges.size() * sizeof(EdgeRec), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.estart, X.estart.data(), X.estart.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_zcell, zc.data(), n * sizeof(double), cudaMemcpyHostToDevice, s));
@@ -454,7 +445,7 @@ int swe_compute_dt(swe_mesh *m, double *dt_out)
 static int launch_steps_direct(swe_mesh *m, int64_t n)
 {
     for (int64_t s = 0; s < n; s++) {
-        swe_step_kernel<<<m->grid, m->block, m->smem, m->stream>>>(m->P, m->cur);
+        swe_step_kernel<<<m->grid, m->block, m->smem, m->stream>>>(m->P, m->cur, 1);
         m->cur ^= 1;
         m->launches++;
     }
@@ -474,7 +465,7 @@ static int graph_for(swe_mesh *m, int steps, cudaGraphExec_t *out)
     cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
     int c = m->cur;
     if (e == cudaSuccess) {
-        for (int s = 0; s < steps; s++) { swe_step_kernel<<<m->grid, m->block, m->smem, cap>>>(m->P, c); c ^= 1; }
+        for (int s = 0; s < steps; s++) { swe_step_kernel<<<m->grid, m->block, m->smem, cap>>>(m->P, c, 1); c ^= 1; }
         e = cudaStreamEndCapture(cap, &g);
     }
     if (e == cudaSuccess) e = cudaGraphInstantiate(&ex, g, 0);
@@ -497,7 +488,7 @@ int swe_run(swe_mesh *m, int64_t nsteps)
     if (m->loop_mode == SWE_LOOP_PERSISTENT) {
         Params P = m->P; int cur = m->cur; long long ns = nsteps;
         void *args[] = { &P, &cur, &ns };
-        CK(cudaLaunchCooperativeKernel((void *)swe_persistent_kernel, dim3(m->coop_grid), dim3(m->block), args, m->smem, m->stream));
+        CK(cudaLaunchCooperativeKernel((void *)swe_step_kernel, dim3(m->coop_grid), dim3(m->block), args, m->smem, m->stream));
         m->launches++;
         m->cur ^= (int)(nsteps & 1);
         return SWE_OK;
