@@ -220,6 +220,9 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
         X.tile_cells = TC;
         X.ntiles = (nt + TC - 1) / TC;
         X.estart.assign((size_t)X.ntiles + 1, 0);
+        X.hstart.assign((size_t)X.ntiles + 1, 0);
+        X.halo.clear(); X.max_halo = 0;
+        std::vector<int32_t> halo_tile((size_t)nt, -1), halo_slot((size_t)nt, 0);
         X.cellc.assign((size_t)X.ntiles * 3 * TC, 1.0);
         X.edges.clear();
         X.edges.reserve((size_t)nt * 7 / 4 + 1024);
@@ -231,7 +234,17 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
         auto enc = [](int64_t p, int k) { return (int32_t)(p | ((int64_t)k << kHostIdBits)); };
         for (int64_t t = 0; t < X.ntiles; t++) {
             const int64_t base = t * TC, nc = std::min<int64_t>(TC, nt - base);
-            const size_t first = X.edges.size();
+            const size_t first = X.edges.size(), hfirst = X.halo.size();
+            // position of internal cell pj in the tile's record array
+            auto pos = [&](int64_t pj) -> int64_t {
+                if (pj >= base && pj < base + TC) return pj - base;
+                if (halo_tile[(size_t)pj] != (int32_t)t) {
+                    halo_tile[(size_t)pj] = (int32_t)t;
+                    halo_slot[(size_t)pj] = (int32_t)(X.halo.size() - hfirst);
+                    X.halo.push_back((int32_t)pj);
+                }
+                return TC + halo_slot[(size_t)pj];
+            };
             double *cc = X.cellc.data() + (size_t)t * 3 * TC;
             for (int64_t q = 0; q < TC; q++) cc[2 * TC + q] = 0.0;
             for (int64_t q = 0; q < nc; q++) {
@@ -241,7 +254,7 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
                     const int32_t j = T.nbr[3 * (size_t)c + k];
                     const double *nk = &T.normal[6 * (size_t)c + 2 * k];
                     if (j < 0) {                                   // boundary edge: a = this cell
-                        X.edges.push_back({ enc(p, k), j, nk[0], nk[1], T.length[3 * (size_t)c + k] });
+                        X.edges.push_back({ enc(q, k), j, nk[0], nk[1], T.length[3 * (size_t)c + k] });
                         continue;
                     }
                     const int64_t pj = T.inv[(size_t)j];
@@ -250,9 +263,9 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
                     const int kj = local_edge_towards(j, c);
                     if (kj < 0) { err = "inconsistent neighbour table"; return SWE_ERR_NON_MANIFOLD; }
                     if (c < j)                                     // a = smaller caller id (R-17)
-                        X.edges.push_back({ enc(p, k), enc(pj, kj), nk[0], nk[1], T.length[3 * (size_t)c + k] });
+                        X.edges.push_back({ enc(q, k), enc(pos(pj), kj), nk[0], nk[1], T.length[3 * (size_t)c + k] });
                     else
-                        X.edges.push_back({ enc(pj, kj), enc(p, k), T.normal[6 * (size_t)j + 2 * kj],
+                        X.edges.push_back({ enc(pos(pj), kj), enc(q, k), T.normal[6 * (size_t)j + 2 * kj],
                                             T.normal[6 * (size_t)j + 2 * kj + 1], T.length[3 * (size_t)j + kj] });
                 }
                 cc[q] = 1.0 / T.area[(size_t)c];
@@ -263,6 +276,10 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
             if (X.edges.size() > (size_t)INT32_MAX) { err = "too many edges"; return SWE_ERR_INVALID_ARG; }
             X.max_edges = std::max<int32_t>(X.max_edges, (int32_t)cnt);
             X.estart[(size_t)t + 1] = (int32_t)X.edges.size();
+            while (X.halo.size() % 4) X.halo.push_back(-1);          // 16-byte granules for the bulk copy
+            if (X.halo.size() > (size_t)INT32_MAX) { err = "too many halo cells"; return SWE_ERR_INVALID_ARG; }
+            X.max_halo = std::max<int32_t>(X.max_halo, (int32_t)(X.halo.size() - hfirst));
+            X.hstart[(size_t)t + 1] = (int32_t)X.halo.size();
         }
     } catch (const std::bad_alloc &) { err = "out of host memory"; return SWE_ERR_NOMEM; }
     return SWE_OK;

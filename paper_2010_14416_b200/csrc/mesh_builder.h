@@ -29,14 +29,18 @@ struct HostTables {
 // Tile tables of the step kernel (swe_kernels.cuh), in the INTERNAL cell numbering: the cells
 // are cut into tiles of tile_cells consecutive cells; every edge that touches a tile appears
 // once in that tile's edge list (an edge between two tiles appears in both lists).
-// Edge end points: internal cell id in bits 0-28, the edge's local index k in that cell in bits
-// 29-30; b = -tag on a boundary edge.  a is the end point with the smaller CALLER id.
+// Edge end points: bits 0-28 = position in the tile's record array (local cell index if
+// < tile_cells, else tile_cells + index into the tile's halo list), bits 29-30 = the edge's local
+// index k in that cell; b = -tag on a boundary edge.  a is the end point with the smaller CALLER id.
 struct HostEdge { int32_t a, b; double n1, n2, len; };                          // 32 bytes
 constexpr int kHostIdBits = 29;
 struct TileTables {
     int32_t tile_cells = 0;
     int64_t ntiles = 0;
     int32_t max_edges = 0;             // longest edge list of any tile
+    int32_t max_halo = 0;              // longest (padded) halo list of any tile
+    std::vector<int32_t> hstart;       // [ntiles + 1] offsets into halo, multiples of 4
+    std::vector<int32_t> halo;         // internal ids of the off-tile end points, -1 = padding
     std::vector<int32_t> estart;       // [ntiles + 1] offsets into edges
     std::vector<HostEdge> edges;
     std::vector<double> cellc;         // [ntiles][3][tile_cells]: 1/|Omega|, 1/R, g m^2 (padded with 1, 1, 0)

@@ -41,8 +41,9 @@ struct __align__(32) Rec { double h, u, v, z; };
 // One edge of a tile.  a is always a cell; b is a cell or -tag on a boundary edge.  (n1,n2) is
 // a's unit outward normal on this edge (so b's is its negative).  a is the end point with the
 // smaller CALLER id, which makes the result independent of the renumbering (R-17).
-// Cell ids are internal ids in bits 0-28; bits 29-30 hold the local edge index k of this edge
-// in that cell.
+// Bits 0-28 of a and b: position in the tile's shared-memory record array (< tile size: the
+// tile's own cell with that local index; >= tile size: entry of the tile's halo list);
+// bits 29-30: the local edge index k of this edge in that cell.
 struct __align__(32) EdgeRec { int32_t a, b; double n1, n2, len; };
 constexpr int kIdBits = 29;
 constexpr int32_t kIdMask = (1 << kIdBits) - 1;
@@ -62,10 +63,12 @@ struct Params {
     const double *cellc;      // [ntiles][3][tile] per tile: 1/|Omega|, 1/R, g m^2 (SoA, padded)
     const EdgeRec *edges;     // [estart[ntiles]] tile after tile
     const int32_t *estart;    // [ntiles + 1]
+    const int32_t *halo;      // [hstart[ntiles]] internal ids of each tile's off-tile end points (-1 = padding)
+    const int32_t *hstart;    // [ntiles + 1], multiples of 4
     const double *qn_tag;     // [128] unit discharge along the outward normal per inflow tag
     double *pmax0, *pmax1;    // [npart] per-block max rate of state U0 / U1
     Ctrl *ctrl;
-    int32_t nt, ntiles, npart, max_edges;
+    int32_t nt, ntiles, npart, max_edges, max_halo;
     double g, inv_g, cfl, hdry;
     // selected with a ternary so the kernel parameter block is never indexed dynamically
     __host__ __device__ __forceinline__ Rec *U(int c) const { return c ? U1 : U0; }
@@ -330,117 +333,187 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned by
                  :: "r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-// ---- the tile pipeline -----------------------------------------------------------------------------
-// Shared memory of one block (dynamic), TC = blockDim.x, ME = P.max_edges:
-//   double  so[9][TC]            (k, component) slots of the tile's cells
-//   per stage s = 0..kStages-1:  Rec srec[TC]; double scell[3][TC]; EdgeRec sedge[ME]
-//   uint64  bar[kStages]
-#ifndef SWE_STAGES
-#define SWE_STAGES 2
-#endif
-constexpr int kStages = SWE_STAGES;   // 2: the next tile's copies fly during this tile's compute
-__host__ __device__ __forceinline__ size_t stage_bytes(int TC, int ME)
+// per-thread asynchronous copies (LDGSTS): no registers, completion by cp.async.wait_group
+__device__ __forceinline__ void cp_async16(void *dst, const void *src)
 {
-    return (size_t)TC * sizeof(Rec) + (size_t)TC * 3 * sizeof(double) + (size_t)ME * sizeof(EdgeRec);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(smem_u32(dst)), "l"(src) : "memory");
 }
-__host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int ME)
+__device__ __forceinline__ void cp_async8(void *dst, const void *src)
 {
-    return (size_t)TC * 9 * sizeof(double) + kStages * stage_bytes(TC, ME) + kStages * sizeof(uint64_t);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait()
+{
+    asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory");
 }
 
+// ---- the tile pipeline -----------------------------------------------------------------------------
+// Shared memory of one block (dynamic); TC = blockDim.x, MH = P.max_halo, ME = P.max_edges:
+//   double  so[9][TC]              (local edge k, component) flux slots of the tile's cells
+//   Rec     srec[2][TC + MH]       state records of the tile's cells, then of its halo cells
+//   EdgeRec sedge[ME]              the tile's edge list
+//   double  scell[3][TC]           1/|Omega|, 1/R, g m^2
+//   int32   shalo[3][MH]           halo id lists (three tiles deep)
+//   uint64  bar[6]                 rec[2], halo[3], edge[1]
+// Schedule for the block's n-th tile (s = n & 1), all copies asynchronous:
+//   top      wait: own halo gathers of tile n, records of tile n, edge list of tile n; barrier
+//            issue: records of tile n+1 (bulk) -> srec[s^1]; halo ids of tile n+2 (bulk);
+//                   cell constants of tile n (cp.async); halo gathers of tile n+1 (cp.async,
+//                   ids landed one tile ago) -> srec[s^1][TC..]
+//   phase 1  edges: shared memory only
+//   mid      barrier; issue: edge list of tile n+1 (bulk) into the single edge buffer
+//   phase 2  cells
 struct TilePipe {
-    double *so; unsigned char *stage0; uint64_t *bar; size_t sbytes;
-    __device__ __forceinline__ Rec *srec(int s) const { return reinterpret_cast<Rec *>(stage0 + s * sbytes); }
-    __device__ __forceinline__ double *scell(int s, int TC) const
-    { return reinterpret_cast<double *>(stage0 + s * sbytes + (size_t)TC * sizeof(Rec)); }
-    __device__ __forceinline__ EdgeRec *sedge(int s, int TC) const
-    { return reinterpret_cast<EdgeRec *>(stage0 + s * sbytes + (size_t)TC * (sizeof(Rec) + 3 * sizeof(double))); }
+    double *so; Rec *srec0; EdgeRec *sedge; double *scell; int32_t *shalo0; uint64_t *bar;
+    int rec_stride, MH;
+    __device__ __forceinline__ Rec *srec(int s) const { return srec0 + s * rec_stride; }
+    __device__ __forceinline__ int32_t *shalo(int j) const { return shalo0 + j * MH; }
+    __device__ __forceinline__ uint64_t *rbar(int s) const { return bar + s; }
+    __device__ __forceinline__ uint64_t *hbar(int j) const { return bar + 2 + j; }
+    __device__ __forceinline__ uint64_t *ebar() const { return bar + 5; }
 };
+constexpr int kNumBars = 6;
+__host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int ME)
+{
+    return (size_t)TC * 9 * sizeof(double) + 2 * (size_t)(TC + MH) * sizeof(Rec) +
+           (size_t)ME * sizeof(EdgeRec) + (size_t)TC * 3 * sizeof(double) +
+           3 * (size_t)MH * sizeof(int32_t) + kNumBars * sizeof(uint64_t);
+}
 __device__ __forceinline__ TilePipe make_pipe(const Params &P, unsigned char *smem)
 {
     const int TC = blockDim.x;
     TilePipe p;
-    p.so = reinterpret_cast<double *>(smem);
-    p.stage0 = smem + (size_t)TC * 9 * sizeof(double);
-    p.sbytes = stage_bytes(TC, P.max_edges);
-    p.bar = reinterpret_cast<uint64_t *>(p.stage0 + kStages * p.sbytes);
+    p.MH = P.max_halo; p.rec_stride = TC + P.max_halo;
+    p.so = reinterpret_cast<double *>(smem);                 smem += (size_t)TC * 9 * sizeof(double);
+    p.srec0 = reinterpret_cast<Rec *>(smem);                 smem += 2 * (size_t)p.rec_stride * sizeof(Rec);
+    p.sedge = reinterpret_cast<EdgeRec *>(smem);             smem += (size_t)P.max_edges * sizeof(EdgeRec);
+    p.scell = reinterpret_cast<double *>(smem);              smem += (size_t)TC * 3 * sizeof(double);
+    p.shalo0 = reinterpret_cast<int32_t *>(smem);            smem += 3 * (size_t)P.max_halo * sizeof(int32_t);
+    p.bar = reinterpret_cast<uint64_t *>(smem);
     return p;
 }
-// one thread: arm the stage's barrier and start the three bulk copies of `tile`
-__device__ __forceinline__ void issue_tile(const Params &P, const TilePipe &pp, const Rec *Uin,
+
+// single-thread issue helpers
+__device__ __forceinline__ void issue_recs(const Params &P, const TilePipe &pp, const Rec *Uin,
                                            const int tile, const int s)
 {
-    const int TC = blockDim.x;
-    const int base = tile * TC, nc = min(TC, P.nt - base);
+    const int TC = blockDim.x, base = tile * TC, nc = min(TC, P.nt - base);
+    mbar_expect_tx(pp.rbar(s), (unsigned)nc * sizeof(Rec));
+    bulk_g2s(pp.srec(s), Uin + base, (unsigned)nc * sizeof(Rec), pp.rbar(s));
+}
+__device__ __forceinline__ void issue_edges(const Params &P, const TilePipe &pp, const int tile)
+{
     const int e0 = __ldg(P.estart + tile), ne = __ldg(P.estart + tile + 1) - e0;
-    const unsigned b_rec = (unsigned)nc * sizeof(Rec), b_cell = (unsigned)TC * 3 * sizeof(double),
-                   b_edge = (unsigned)ne * sizeof(EdgeRec);
-    mbar_expect_tx(pp.bar + s, b_rec + b_cell + b_edge);
-    bulk_g2s(pp.srec(s), Uin + base, b_rec, pp.bar + s);
-    bulk_g2s(pp.scell(s, TC), P.cellc + (size_t)tile * 3 * TC, b_cell, pp.bar + s);
-    bulk_g2s(pp.sedge(s, TC), P.edges + e0, b_edge, pp.bar + s);
+    mbar_expect_tx(pp.ebar(), (unsigned)ne * sizeof(EdgeRec));
+    bulk_g2s(pp.sedge, P.edges + e0, (unsigned)ne * sizeof(EdgeRec), pp.ebar());
+}
+// halo lists are padded to a multiple of 4 ids (16 bytes); an empty list still completes a phase
+__device__ __forceinline__ void issue_halo_ids(const Params &P, const TilePipe &pp, const int tile,
+                                               const int j)
+{
+    const int h0 = __ldg(P.hstart + tile), nh = __ldg(P.hstart + tile + 1) - h0;
+    if (nh > 0) {
+        mbar_expect_tx(pp.hbar(j), (unsigned)nh * sizeof(int32_t));
+        bulk_g2s(pp.shalo(j), P.halo + h0, (unsigned)nh * sizeof(int32_t), pp.hbar(j));
+    } else {
+        asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(pp.hbar(j))) : "memory");
+    }
+}
+// all threads: gather the halo records of `tile` (ids in shalo[j]) into srec[s][TC..]
+__device__ __forceinline__ void gather_halo(const Params &P, const TilePipe &pp, const Rec *Uin,
+                                            const int tile, const int j, const int s)
+{
+    const int TC = blockDim.x;
+    const int nh = __ldg(P.hstart + tile + 1) - __ldg(P.hstart + tile);
+    const int32_t *ids = pp.shalo(j);
+    Rec *dst = pp.srec(s) + TC;
+    for (int q = threadIdx.x; q < nh; q += TC) {
+        const int32_t id = ids[q];
+        if (id >= 0) {                                   // padding entries are -1
+            const char *src = reinterpret_cast<const char *>(Uin + id);
+            cp_async16(reinterpret_cast<char *>(dst + q), src);
+            cp_async16(reinterpret_cast<char *>(dst + q) + 16, src + 16);
+        }
+    }
 }
 
-// All the tiles of this block for one time step.  `it0` = number of tiles this block has pushed
-// through the pipeline before (persistent loop), which fixes stage and barrier parity.
-// Returns the block-local maximum rate contribution of this thread.
+// All the tiles of this block for one time step.  `n0` = number of tiles this block has pushed
+// through the pipeline before (persistent loop), which fixes the buffers and barrier parities.
+// Returns this thread's maximum rate contribution.
 __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe &pp,
                                              const Rec *__restrict__ Uin, Rec *__restrict__ Uout,
-                                             const double dt, unsigned &nclamp, unsigned &it0)
+                                             const double dt, unsigned &nclamp, unsigned &n0)
 {
-    const int TC = blockDim.x, tid = threadIdx.x;
+    const int TC = blockDim.x, tid = threadIdx.x, G = gridDim.x;
     double rate = 0.0;
-    unsigned it = it0;
+    unsigned n = n0;
     int tile = blockIdx.x;
     if (tile >= P.ntiles) return 0.0;
-    if (kStages > 1 && tid == 0) issue_tile(P, pp, Uin, tile, it % kStages);
-    for (; tile < P.ntiles; tile += gridDim.x, it++) {
-        const int s = it % kStages;
+    // ---- prologue: everything tile n needs, and the halo ids of tile n+1
+    if (tid == 0) {
+        issue_halo_ids(P, pp, tile, n % 3);
+        issue_recs(P, pp, Uin, tile, n & 1);
+        issue_edges(P, pp, tile);
+        if (tile + G < P.ntiles) issue_halo_ids(P, pp, tile + G, (n + 1) % 3);
+    }
+    mbar_wait(pp.hbar(n % 3), (n / 3) & 1u);
+    gather_halo(P, pp, Uin, tile, n % 3, n & 1);
+    cp_async_commit();
+    for (; tile < P.ntiles; tile += G, n++) {
+        const int s = n & 1;
         const int base = tile * TC;
         const int ne = __ldg(P.estart + tile + 1) - __ldg(P.estart + tile);
-        if (kStages > 1) {
-            mbar_wait(pp.bar + s, (it / kStages) & 1u);
-            __syncthreads();      // every thread has left the previous tile: so[] and the other stage are free
-            if (tid == 0 && tile + (int)gridDim.x < P.ntiles)
-                issue_tile(P, pp, Uin, tile + gridDim.x, (it + 1) % kStages);
-        } else {
-            __syncthreads();
-            if (tid == 0) issue_tile(P, pp, Uin, tile, 0);
-            mbar_wait(pp.bar, it & 1u);
+        const bool have_next = tile + G < P.ntiles;
+        // ---- top
+        cp_async_wait<0>();                               // own halo gathers of this tile
+        mbar_wait(pp.rbar(s), (n >> 1) & 1u);
+        mbar_wait(pp.ebar(), n & 1u);
+        __syncthreads();     // everyone has left the previous tile; everyone's gathers are visible
+        if (tid == 0 && have_next) {
+            issue_recs(P, pp, Uin, tile + G, s ^ 1);
+            if (tile + 2 * G < P.ntiles) issue_halo_ids(P, pp, tile + 2 * G, (n + 2) % 3);
         }
+        if (base + tid < P.nt) {
+            const double *src = P.cellc + (size_t)tile * 3 * TC + tid;
+            double *dst = pp.scell + tid;
+            cp_async8(dst, src); cp_async8(dst + TC, src + TC); cp_async8(dst + 2 * TC, src + 2 * TC);
+        }
+        cp_async_commit();
+        if (have_next) {
+            mbar_wait(pp.hbar((n + 1) % 3), ((n + 1) / 3) & 1u);
+            gather_halo(P, pp, Uin, tile + G, (n + 1) % 3, s ^ 1);
+        }
+        cp_async_commit();
         const Rec *srec = pp.srec(s);
-        const EdgeRec *sedge = pp.sedge(s, TC);
         double *so = pp.so;
-        // ---- phase 1: every edge of the tile once
+        // ---- phase 1: every edge of the tile once, shared memory only
         for (int e = tid; e < ne; e += TC) {
-            const EdgeRec er = sedge[e];
-            const int ia = (er.a & kIdMask) - base, ka = er.a >> kIdBits;
-            const bool inA = (unsigned)ia < (unsigned)TC;
-            Rec A, B;
-            if (inA) A = srec[ia]; else A = load_rec(Uin + (er.a & kIdMask));
-            int ib = -1, kb = 0; bool inB = false;
-            if (er.b >= 0) {
-                ib = (er.b & kIdMask) - base; kb = er.b >> kIdBits;
-                inB = (unsigned)ib < (unsigned)TC;
-                if (inB) B = srec[ib]; else B = load_rec(Uin + (er.b & kIdMask));
-            }
+            const EdgeRec er = pp.sedge[e];
+            const int ia = er.a & kIdMask, ka = er.a >> kIdBits;
+            const Rec A = srec[ia];
+            Rec B;
+            int ib = TC, kb = 0;
+            if (er.b >= 0) { ib = er.b & kIdMask; kb = er.b >> kIdBits; B = srec[ib]; }
             double o[5];
             edge_eval(P, er, A, B, o);
-            if (inA) {
+            if (ia < TC) {
                 double *q = so + (ka * 3) * TC + ia;
                 q[0] = o[0]; q[TC] = o[1]; q[2 * TC] = o[2];
             }
-            if (inB) {
+            if (ib < TC) {
                 double *q = so + (kb * 3) * TC + ib;
                 q[0] = -o[0]; q[TC] = -o[3]; q[2 * TC] = -o[4];
             }
         }
+        cp_async_wait<1>();                               // this tile's cell constants
         __syncthreads();
+        if (tid == 0 && have_next) issue_edges(P, pp, tile + G);
         // ---- phase 2: every cell of the tile
         const int i = base + tid;
         if (i < P.nt) {
             const Rec Ui = srec[tid];
-            const double *sc = pp.scell(s, TC) + tid;
+            const double *sc = pp.scell + tid;
             const double *q = so + tid;
             // three edges in the fixed order k = 0,1,2 (R-17)
             const double s1 = (q[0] + q[3 * TC]) + q[6 * TC];
@@ -451,7 +524,8 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe &pp
             store_rec(Uout + i, Un);
         }
     }
-    it0 = it;
+    cp_async_wait<0>();
+    n0 = n;
     return rate;
 }
 

@@ -31,7 +31,7 @@ __device__ __forceinline__ TilePipe pipe_setup(const Params &P)
 {
     const TilePipe pp = make_pipe(P, dyn_smem);
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kStages; s++) mbar_init(pp.bar + s, 1);
+        for (int s = 0; s < kNumBars; s++) mbar_init(pp.bar + s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -166,7 +166,7 @@ static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 namespace {
 static_assert(sizeof(HostEdge) == sizeof(EdgeRec) && kHostIdBits == kIdBits, "table records");
 struct Layout {
-    size_t U0, U1, cellc, edges, estart, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
+    size_t U0, U1, cellc, edges, estart, halo, hstart, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
 };
 Layout make_layout(const HostTables &T, const TileTables &X)
 {
@@ -175,6 +175,7 @@ Layout make_layout(const HostTables &T, const TileTables &X)
     L.U0 = take(n * sizeof(Rec)); L.U1 = take(n * sizeof(Rec));
     L.cellc = take(X.cellc.size() * sizeof(double)); L.edges = take(X.edges.size() * sizeof(EdgeRec));
     L.estart = take(X.estart.size() * sizeof(int32_t));
+    L.halo = take(X.halo.size() * sizeof(int32_t) + 16); L.hstart = take(X.hstart.size() * sizeof(int32_t));
     L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
     L.stage = take(3 * n * sizeof(double));
     L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
@@ -295,9 +296,9 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     CK(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
     CK(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-    // dynamic shared memory: flux slots + two stages of {state records, cell constants, longest edge list}
+    // dynamic shared memory of the tile pipeline (swe_kernels.cuh), sized for this mesh's longest lists
     const TileTables &X = m->X;
-    m->smem = tile_smem_bytes(m->block, X.max_edges);
+    m->smem = tile_smem_bytes(m->block, X.max_halo, X.max_edges);
     if (m->smem > (size_t)smem_optin) { m->err = "tile does not fit in shared memory"; return SWE_ERR_CUDA; }
     CK(cudaFuncSetAttribute(swe_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem));
     int occ_step = 0, occ_pers = 0;
@@ -318,12 +319,13 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.U0 = (Rec *)(m->ws + L.U0); P.U1 = (Rec *)(m->ws + L.U1);
     P.cellc = (const double *)(m->ws + L.cellc); P.edges = (const EdgeRec *)(m->ws + L.edges);
     P.estart = (const int32_t *)(m->ws + L.estart);
+    P.halo = (const int32_t *)(m->ws + L.halo); P.hstart = (const int32_t *)(m->ws + L.hstart);
     m->d_zcell = (double *)(m->ws + L.zcell); m->d_perm = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
     m->d_qn = (double *)(m->ws + L.qn); P.qn_tag = m->d_qn;
     P.ctrl = (Ctrl *)(m->ws + L.ctrl);
-    P.nt = (int32_t)T.nt; P.ntiles = ntiles; P.max_edges = X.max_edges;
+    P.nt = (int32_t)T.nt; P.ntiles = ntiles; P.max_edges = X.max_edges; P.max_halo = X.max_halo;
     P.npart = mode == SWE_LOOP_PERSISTENT ? m->coop_grid : m->grid;
     P.g = m->prm.g; P.inv_g = 1.0 / m->prm.g; P.cfl = m->prm.cfl;
     // a side is dry iff h <= h_dry; the floor keeps every argument of the MUFU-seeded
@@ -337,6 +339,8 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
         CK(cudaMemcpyAsync(m->ws + L.cellc, X.cellc.data(), X.cellc.size() * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.edges, X.edges.data(), X.edges.size() * sizeof(EdgeRec), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.estart, X.estart.data(), X.estart.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        if (!X.halo.empty()) CK(cudaMemcpyAsync(m->ws + L.halo, X.halo.data(), X.halo.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.hstart, X.hstart.data(), X.hstart.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_zcell, zc.data(), n * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_perm, T.perm.data(), n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_qn, m->qn_tag, sizeof(m->qn_tag), cudaMemcpyHostToDevice, s));
