@@ -220,8 +220,8 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
         X.tile_cells = TC;
         X.ntiles = (nt + TC - 1) / TC;
         X.estart.assign((size_t)X.ntiles + 1, 0);
-        X.hstart.assign((size_t)X.ntiles + 1, 0);
-        X.halo.clear(); X.max_halo = 0;
+        std::vector<int32_t> hstart((size_t)X.ntiles + 1, 0), halo;
+        X.max_halo = 0;
         std::vector<int32_t> halo_tile((size_t)nt, -1), halo_slot((size_t)nt, 0);
         X.cellc.assign((size_t)X.ntiles * 3 * TC, 1.0);
         X.edges.clear();
@@ -234,14 +234,14 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
         auto enc = [](int64_t p, int k) { return (int32_t)(p | ((int64_t)k << kHostIdBits)); };
         for (int64_t t = 0; t < X.ntiles; t++) {
             const int64_t base = t * TC, nc = std::min<int64_t>(TC, nt - base);
-            const size_t first = X.edges.size(), hfirst = X.halo.size();
+            const size_t first = X.edges.size(), hfirst = halo.size();
             // position of internal cell pj in the tile's record array
             auto pos = [&](int64_t pj) -> int64_t {
                 if (pj >= base && pj < base + TC) return pj - base;
                 if (halo_tile[(size_t)pj] != (int32_t)t) {
                     halo_tile[(size_t)pj] = (int32_t)t;
-                    halo_slot[(size_t)pj] = (int32_t)(X.halo.size() - hfirst);
-                    X.halo.push_back((int32_t)pj);
+                    halo_slot[(size_t)pj] = (int32_t)(halo.size() - hfirst);
+                    halo.push_back((int32_t)pj);
                 }
                 return TC + halo_slot[(size_t)pj];
             };
@@ -276,10 +276,20 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
             if (X.edges.size() > (size_t)INT32_MAX) { err = "too many edges"; return SWE_ERR_INVALID_ARG; }
             X.max_edges = std::max<int32_t>(X.max_edges, (int32_t)cnt);
             X.estart[(size_t)t + 1] = (int32_t)X.edges.size();
-            while (X.halo.size() % 4) X.halo.push_back(-1);          // 16-byte granules for the bulk copy
-            if (X.halo.size() > (size_t)INT32_MAX) { err = "too many halo cells"; return SWE_ERR_INVALID_ARG; }
-            X.max_halo = std::max<int32_t>(X.max_halo, (int32_t)(X.halo.size() - hfirst));
-            X.hstart[(size_t)t + 1] = (int32_t)X.halo.size();
+            if (halo.size() > (size_t)INT32_MAX) { err = "too many halo cells"; return SWE_ERR_INVALID_ARG; }
+            X.max_halo = std::max<int32_t>(X.max_halo, (int32_t)(halo.size() - hfirst));
+            hstart[(size_t)t + 1] = (int32_t)halo.size();
+        }
+        // fixed-stride info blocks (16-byte granules for the bulk copy)
+        X.max_halo = (X.max_halo + 3) / 4 * 4;
+        const size_t stride = 4 + (size_t)X.max_halo;
+        X.tinfo.assign((size_t)X.ntiles * stride, -1);
+        for (int64_t t = 0; t < X.ntiles; t++) {
+            int32_t *ti = X.tinfo.data() + (size_t)t * stride;
+            const int32_t nh = hstart[(size_t)t + 1] - hstart[(size_t)t];
+            ti[0] = X.estart[(size_t)t]; ti[1] = X.estart[(size_t)t + 1] - X.estart[(size_t)t];
+            ti[2] = nh; ti[3] = 0;
+            std::copy(halo.begin() + hstart[(size_t)t], halo.begin() + hstart[(size_t)t + 1], ti + 4);
         }
     } catch (const std::bad_alloc &) { err = "out of host memory"; return SWE_ERR_NOMEM; }
     return SWE_OK;

@@ -38,9 +38,10 @@ struct TileTables {
     int32_t tile_cells = 0;
     int64_t ntiles = 0;
     int32_t max_edges = 0;             // longest edge list of any tile
-    int32_t max_halo = 0;              // longest (padded) halo list of any tile
-    std::vector<int32_t> hstart;       // [ntiles + 1] offsets into halo, multiples of 4
-    std::vector<int32_t> halo;         // internal ids of the off-tile end points, -1 = padding
+    int32_t max_halo = 0;              // longest halo list of any tile, rounded up to a multiple of 4
+    // [ntiles][4 + max_halo]: {first edge, #edges, #halo ids, 0, halo ids (internal cell ids of the
+    // tile's off-tile end points) padded with -1}
+    std::vector<int32_t> tinfo;
     std::vector<int32_t> estart;       // [ntiles + 1] offsets into edges
     std::vector<HostEdge> edges;
     std::vector<double> cellc;         // [ntiles][3][tile_cells]: 1/|Omega|, 1/R, g m^2 (padded with 1, 1, 0)

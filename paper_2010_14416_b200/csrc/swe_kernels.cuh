@@ -62,14 +62,12 @@ struct Params {
     Rec *U0, *U1;             // ping-pong state, internal order
     const double *cellc;      // [ntiles][3][tile] per tile: 1/|Omega|, 1/R, g m^2 (SoA, padded)
     const EdgeRec *edges;     // [estart[ntiles]] tile after tile
-    const int32_t *estart;    // [ntiles + 1]
-    const int32_t *halo;      // [hstart[ntiles]] internal ids of each tile's off-tile end points (-1 = padding)
-    const int32_t *hstart;    // [ntiles + 1], multiples of 4
+    const int32_t *tinfo;     // [ntiles][4 + max_halo] per-tile info block, see "the tile pipeline"
     const double *qn_tag;     // [128] unit discharge along the outward normal per inflow tag
     double *pmax0, *pmax1;    // [npart] per-block max rate of state U0 / U1
     Ctrl *ctrl;
     int32_t nt, ntiles, npart, max_edges, max_halo;
-    double g, inv_g, cfl, hdry;
+    double g, hg, inv_g, cfl, hdry;   // hg = g/2
     // selected with a ternary so the kernel parameter block is never indexed dynamically
     __host__ __device__ __forceinline__ Rec *U(int c) const { return c ? U1 : U0; }
     __host__ __device__ __forceinline__ double *pmax(int c) const { return c ? pmax1 : pmax0; }
@@ -155,53 +153,54 @@ __device__ __forceinline__ double reduce_dt(const Params &P, const double *pmax,
 // ---- HLLC flux in the edge frame, eq.(17)-(26) --------------------------------
 // Inputs: reconstructed depths, normal/tangential velocities.  Output (G0,G1,G2) = mass, normal
 // and tangential momentum flux.  Same expression trees as the oracle's step list (DESIGN.md
-// section 4) except that a_k = sqrt(g h_k) and 1/h_k both come from one rsqrt(g h_k), and that
-// a_k p_k of eq.(19)-(20) is formed as sqrt(g h* (h*+h_k) / (2 h_k)) (one square root, R-7).
-__device__ __forceinline__ void hllc_flux(const double g, const double inv_g, const double hdry,
-                                          double hL, double uL, double vL, double hR, double uR,
-                                          double vR, double &G0, double &G1, double &G2)
+// section 4) except that
+//   - a_k = sqrt(g h_k) and 1/h_k both come from one rsqrt(g h_k);
+//   - a_k p_k of eq.(19)-(20) is formed as sqrt(g m (m+h_k) / (2 h_k)) with m = max(h*, h_k):
+//     one square root, and no branch because the formula gives a_k at m = h_k (R-7 continuity).
+// hg = g/2.
+__device__ __forceinline__ void hllc_flux(const double g, const double hg, const double inv_g,
+                                          const double hdry, double hL, double uL, double vL,
+                                          double hR, double uR, double vR, const double pL,
+                                          const double pR, double &G0, double &G1, double &G2)
 {
     const bool dL = hL <= hdry, dR = hR <= hdry;           // R-15
     G0 = 0.0; G1 = 0.0; G2 = 0.0;
     if (dL && dR) return;
-    double SL, SR;
+    double SL, SR, GL1 = pL, GR1 = pR;                      // pressure parts g h^2 / 2
     if (dL) {                                               // eq.(26) line 1
-        hL = 0.0; uL = 0.0; vL = 0.0;
+        hL = 0.0; uL = 0.0; vL = 0.0; GL1 = 0.0;
         const double ghR = g * hR, aR = ghR * fast_rsqrt(ghR);
         SL = uR - 2.0 * aR; SR = uR + aR;
     } else if (dR) {                                        // eq.(26) line 2 (R-18)
-        hR = 0.0; uR = 0.0; vR = 0.0;
+        hR = 0.0; uR = 0.0; vR = 0.0; GR1 = 0.0;
         const double ghL = g * hL, aL = ghL * fast_rsqrt(ghL);
         SL = uL - aL; SR = uL + 2.0 * aL;
     } else {
         const double ghL = g * hL, ghR = g * hR;
         const double rL = fast_rsqrt(ghL), rR = fast_rsqrt(ghR);
         const double aL = ghL * rL, aR = ghR * rR;
-        const double hs_sum = hL + hR, as_sum = aR + aL;
-        const double h0 = 0.5 * hs_sum - (uR - uL) * hs_sum * (0.25 * fast_rcp(as_sum)); // eq.(21)
+        const double ihL = g * (rL * rL), ihR = g * (rR * rR);          // 1/h_k
+        const double hsum = hL + hR, asum = aR + aL, du = uL - uR;
+        const double h0 = fma(du * hsum, 0.25 * fast_rcp(asum), 0.5 * hsum);   // eq.(21)
         double hs;
         if (h0 <= fmin(hL, hR)) {                           // rarefaction, eq.(22), R-6
-            const double w = fmax(0.5 * as_sum + 0.25 * (uL - uR), 0.0);
+            const double w = fmax(fma(0.25, du, 0.5 * asum), 0.0);
             hs = w * w * inv_g;
         } else {                                            // shock, eq.(23)
-            const double k0 = 0.5 * g * fast_rcp(h0);       // g / (2 h0)
-            const double xL = k0 * (h0 + hL) * (g * rL * rL);   // g (h0+hL) / (2 h0 hL)
-            const double xR = k0 * (h0 + hR) * (g * rR * rR);
+            const double k0 = hg * fast_rcp(h0);            // g / (2 h0)
+            const double xL = k0 * (h0 + hL) * ihL;         // g (h0+hL) / (2 h0 hL)
+            const double xR = k0 * (h0 + hR) * ihR;
             const double gL = xL * fast_rsqrt(xL), gR = xR * fast_rsqrt(xR);
-            hs = ((hL * gL + hR * gR) + (uL - uR)) * fast_rcp(gL + gR);
+            hs = ((hL * gL + hR * gR) + du) * fast_rcp(gL + gR);
         }
-        SL = uL - aL; SR = uR + aR;                         // eq.(19) with p_k = 1
-        if (hs > hL) {                                      // eq.(20), R-7
-            const double x = 0.5 * g * hs * (hs + hL) * (g * rL * rL);
-            SL = uL - x * fast_rsqrt(x);
-        }
-        if (hs > hR) {
-            const double x = 0.5 * g * hs * (hs + hR) * (g * rR * rR);
-            SR = uR + x * fast_rsqrt(x);
-        }
+        // eq.(19)-(20), R-7
+        const double mL = fmax(hs, hL), mR = fmax(hs, hR);
+        const double yL = hg * mL * (mL + hL) * ihL, yR = hg * mR * (mR + hR) * ihR;
+        SL = uL - yL * fast_rsqrt(yL);
+        SR = uR + yR * fast_rsqrt(yR);
     }
     const double qL = hL * uL, qR = hR * uR;
-    const double GL1 = qL * uL + 0.5 * g * hL * hL, GR1 = qR * uR + 0.5 * g * hR * hR;
+    GL1 = fma(qL, uL, GL1); GR1 = fma(qR, uR, GR1);
     if (SL >= 0.0) { G0 = qL; G1 = GL1; G2 = qL * vL; return; }                  // eq.(17), R-11
     if (SR <= 0.0) { G0 = qR; G1 = GR1; G2 = qR * vR; return; }
     const double inv = fast_rcp(SR - SL);
@@ -220,24 +219,25 @@ __device__ __forceinline__ void hllc_flux(const double g, const double inv_g, co
 __device__ __forceinline__ void edge_eval(const Params &P, const EdgeRec &er, const Rec &A,
                                           const Rec &B, double o[5])
 {
-    const double g = P.g, hdry = P.hdry;
+    const double g = P.g, hg = P.hg, hdry = P.hdry;
     const double n1 = er.n1, n2 = er.n2;
-    const double uL = A.u * n1 + A.v * n2, vL = A.v * n1 - A.u * n2;             // eq.(12)
+    const double uL = fma(A.u, n1, A.v * n2), vL = fma(A.v, n1, -(A.u * n2));    // eq.(12)
     double G0, G1, G2, sba = 0.0, sbb = 0.0;
     if (er.b >= 0) {
         // a2: hydrostatic reconstruction, eq.(28), R-14
         const double zf = fmax(A.z, B.z);
         const double hL = fmax(0.0, A.h + (A.z - zf));
         const double hR = fmax(0.0, B.h + (B.z - zf));
-        const double uR = B.u * n1 + B.v * n2, vR = B.v * n1 - B.u * n2;
-        hllc_flux(g, P.inv_g, hdry, hL, uL, vL, hR, uR, vR, G0, G1, G2);
+        const double uR = fma(B.u, n1, B.v * n2), vR = fma(B.v, n1, -(B.u * n2));
+        const double hL2 = hL * hL, hR2 = hR * hR;
+        hllc_flux(g, hg, P.inv_g, hdry, hL, uL, vL, hR, uR, vR, hg * hL2, hg * hR2, G0, G1, G2);
         // bathymetry source eq.(30) with g/2 (R-13), one value per side
-        sba = 0.5 * g * (hL * hL - A.h * A.h);
-        sbb = 0.5 * g * (hR * hR - B.h * B.h);
+        sba = hg * (hL2 - A.h * A.h);
+        sbb = hg * (hR2 - B.h * B.h);
     } else {                                    // a6: boundary edge
         const int tag = -er.b;
         const double hL = A.h;
-        const double pr = 0.5 * g * hL * hL;
+        const double pr = hg * hL * hL;
         if (tag == SWE_BC_WALL) { G0 = 0.0; G1 = pr; G2 = 0.0; }                 // R-4
         else if (tag == SWE_BC_TRANSMISSIVE) {                                    // R-21
             if (hL > hdry) { G0 = hL * uL; G1 = G0 * uL + pr; G2 = G0 * vL; }
@@ -251,9 +251,10 @@ __device__ __forceinline__ void edge_eval(const Params &P, const EdgeRec &er, co
     // a7: rotate back (T^-1) and scale by the edge length
     const double L = er.len;
     const double Fx = G1 * n1 - G2 * n2, Fy = G1 * n2 + G2 * n1;
+    const double Ln1 = L * n1, Ln2 = L * n2, LFx = L * Fx, LFy = L * Fy;
     o[0] = L * G0;
-    o[1] = L * (Fx - sba * n1); o[2] = L * (Fy - sba * n2);
-    o[3] = L * (Fx - sbb * n1); o[4] = L * (Fy - sbb * n2);
+    o[1] = fma(-sba, Ln1, LFx); o[2] = fma(-sba, Ln2, LFy);
+    o[3] = fma(-sbb, Ln1, LFx); o[4] = fma(-sbb, Ln2, LFy);
 }
 
 // ---- one cell: a7-a10, eq.(37), PAPER.md:250 ---------------------------------------------------
@@ -349,121 +350,118 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 }
 
 // ---- the tile pipeline -----------------------------------------------------------------------------
-// Shared memory of one block (dynamic); TC = blockDim.x, MH = P.max_halo, ME = P.max_edges:
+// Per-tile info block in global memory (P.tinfo, fixed stride 4 + MH int32, MH = P.max_halo):
+//   [0] first edge of the tile in P.edges   [1] number of edges   [2] number of halo ids
+//   [3] reserved                            [4..] halo ids (internal cell ids), padded with -1
+// Shared memory of one block (dynamic); TC = blockDim.x, ME = P.max_edges:
 //   double  so[9][TC]              (local edge k, component) flux slots of the tile's cells
 //   Rec     srec[2][TC + MH]       state records of the tile's cells, then of its halo cells
 //   EdgeRec sedge[ME]              the tile's edge list
 //   double  scell[3][TC]           1/|Omega|, 1/R, g m^2
-//   int32   shalo[3][MH]           halo id lists (three tiles deep)
-//   uint64  bar[6]                 rec[2], halo[3], edge[1]
+//   int32   sinfo[3][4 + MH]       info blocks (three tiles deep)
+//   uint64  bar[6]                 rec[2], info[3], edge[1]
 // Schedule for the block's n-th tile (s = n & 1), all copies asynchronous:
 //   top      wait: own halo gathers of tile n, records of tile n, edge list of tile n; barrier
-//            issue: records of tile n+1 (bulk) -> srec[s^1]; halo ids of tile n+2 (bulk);
+//            issue: records of tile n+1 (bulk) -> srec[s^1]; info block of tile n+2 (bulk);
 //                   cell constants of tile n (cp.async); halo gathers of tile n+1 (cp.async,
-//                   ids landed one tile ago) -> srec[s^1][TC..]
+//                   its info block landed one tile ago) -> srec[s^1][TC..]
 //   phase 1  edges: shared memory only
 //   mid      barrier; issue: edge list of tile n+1 (bulk) into the single edge buffer
 //   phase 2  cells
-struct TilePipe {
-    double *so; Rec *srec0; EdgeRec *sedge; double *scell; int32_t *shalo0; uint64_t *bar;
-    int rec_stride, MH;
-    __device__ __forceinline__ Rec *srec(int s) const { return srec0 + s * rec_stride; }
-    __device__ __forceinline__ int32_t *shalo(int j) const { return shalo0 + j * MH; }
-    __device__ __forceinline__ uint64_t *rbar(int s) const { return bar + s; }
-    __device__ __forceinline__ uint64_t *hbar(int j) const { return bar + 2 + j; }
-    __device__ __forceinline__ uint64_t *ebar() const { return bar + 5; }
-};
+constexpr int kInfoHdr = 4;
 constexpr int kNumBars = 6;
 __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int ME)
 {
     return (size_t)TC * 9 * sizeof(double) + 2 * (size_t)(TC + MH) * sizeof(Rec) +
            (size_t)ME * sizeof(EdgeRec) + (size_t)TC * 3 * sizeof(double) +
-           3 * (size_t)MH * sizeof(int32_t) + kNumBars * sizeof(uint64_t);
+           3 * (size_t)(kInfoHdr + MH) * sizeof(int32_t) + kNumBars * sizeof(uint64_t);
 }
-__device__ __forceinline__ TilePipe make_pipe(const Params &P, unsigned char *smem)
+template <int TC> struct TilePipe {
+    double *so; Rec *srec0; EdgeRec *sedge; double *scell; int32_t *sinfo0; uint64_t *bar;
+    int rec_stride, info_stride;
+    __device__ __forceinline__ Rec *srec(int s) const { return srec0 + s * rec_stride; }
+    __device__ __forceinline__ int32_t *sinfo(int j) const { return sinfo0 + j * info_stride; }
+    __device__ __forceinline__ uint64_t *rbar(int s) const { return bar + s; }
+    __device__ __forceinline__ uint64_t *ibar(int j) const { return bar + 2 + j; }
+    __device__ __forceinline__ uint64_t *ebar() const { return bar + 5; }
+};
+template <int TC> __device__ __forceinline__ TilePipe<TC> make_pipe(const Params &P, unsigned char *smem)
 {
-    const int TC = blockDim.x;
-    TilePipe p;
-    p.MH = P.max_halo; p.rec_stride = TC + P.max_halo;
+    TilePipe<TC> p;
+    p.rec_stride = TC + P.max_halo; p.info_stride = kInfoHdr + P.max_halo;
     p.so = reinterpret_cast<double *>(smem);                 smem += (size_t)TC * 9 * sizeof(double);
     p.srec0 = reinterpret_cast<Rec *>(smem);                 smem += 2 * (size_t)p.rec_stride * sizeof(Rec);
     p.sedge = reinterpret_cast<EdgeRec *>(smem);             smem += (size_t)P.max_edges * sizeof(EdgeRec);
     p.scell = reinterpret_cast<double *>(smem);              smem += (size_t)TC * 3 * sizeof(double);
-    p.shalo0 = reinterpret_cast<int32_t *>(smem);            smem += 3 * (size_t)P.max_halo * sizeof(int32_t);
+    p.sinfo0 = reinterpret_cast<int32_t *>(smem);            smem += 3 * (size_t)p.info_stride * sizeof(int32_t);
     p.bar = reinterpret_cast<uint64_t *>(smem);
     return p;
 }
 
 // single-thread issue helpers
-__device__ __forceinline__ void issue_recs(const Params &P, const TilePipe &pp, const Rec *Uin,
-                                           const int tile, const int s)
+template <int TC> __device__ __forceinline__ void issue_recs(const Params &P, const TilePipe<TC> &pp,
+                                                             const Rec *Uin, const int tile, const int s)
 {
-    const int TC = blockDim.x, base = tile * TC, nc = min(TC, P.nt - base);
+    const int base = tile * TC, nc = min(TC, P.nt - base);
     mbar_expect_tx(pp.rbar(s), (unsigned)nc * sizeof(Rec));
     bulk_g2s(pp.srec(s), Uin + base, (unsigned)nc * sizeof(Rec), pp.rbar(s));
 }
-__device__ __forceinline__ void issue_edges(const Params &P, const TilePipe &pp, const int tile)
+template <int TC> __device__ __forceinline__ void issue_edges(const Params &P, const TilePipe<TC> &pp,
+                                                              const int e0, const int ne)
 {
-    const int e0 = __ldg(P.estart + tile), ne = __ldg(P.estart + tile + 1) - e0;
     mbar_expect_tx(pp.ebar(), (unsigned)ne * sizeof(EdgeRec));
     bulk_g2s(pp.sedge, P.edges + e0, (unsigned)ne * sizeof(EdgeRec), pp.ebar());
 }
-// halo lists are padded to a multiple of 4 ids (16 bytes); an empty list still completes a phase
-__device__ __forceinline__ void issue_halo_ids(const Params &P, const TilePipe &pp, const int tile,
-                                               const int j)
+template <int TC> __device__ __forceinline__ void issue_info(const Params &P, const TilePipe<TC> &pp,
+                                                             const int tile, const int j)
 {
-    const int h0 = __ldg(P.hstart + tile), nh = __ldg(P.hstart + tile + 1) - h0;
-    if (nh > 0) {
-        mbar_expect_tx(pp.hbar(j), (unsigned)nh * sizeof(int32_t));
-        bulk_g2s(pp.shalo(j), P.halo + h0, (unsigned)nh * sizeof(int32_t), pp.hbar(j));
-    } else {
-        asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(smem_u32(pp.hbar(j))) : "memory");
-    }
+    const unsigned bytes = (unsigned)pp.info_stride * sizeof(int32_t);
+    mbar_expect_tx(pp.ibar(j), bytes);
+    bulk_g2s(pp.sinfo(j), P.tinfo + (size_t)tile * pp.info_stride, bytes, pp.ibar(j));
 }
-// all threads: gather the halo records of `tile` (ids in shalo[j]) into srec[s][TC..]
-__device__ __forceinline__ void gather_halo(const Params &P, const TilePipe &pp, const Rec *Uin,
-                                            const int tile, const int j, const int s)
+// all threads: gather the halo records listed in info block j into srec[s][TC..]
+template <int TC> __device__ __forceinline__ void gather_halo(const TilePipe<TC> &pp, const Rec *Uin,
+                                                              const int j, const int s)
 {
-    const int TC = blockDim.x;
-    const int nh = __ldg(P.hstart + tile + 1) - __ldg(P.hstart + tile);
-    const int32_t *ids = pp.shalo(j);
+    const int32_t *info = pp.sinfo(j);
+    const int nh = info[2];
     Rec *dst = pp.srec(s) + TC;
     for (int q = threadIdx.x; q < nh; q += TC) {
-        const int32_t id = ids[q];
-        if (id >= 0) {                                   // padding entries are -1
-            const char *src = reinterpret_cast<const char *>(Uin + id);
-            cp_async16(reinterpret_cast<char *>(dst + q), src);
-            cp_async16(reinterpret_cast<char *>(dst + q) + 16, src + 16);
-        }
+        const char *src = reinterpret_cast<const char *>(Uin + info[kInfoHdr + q]);
+        cp_async16(reinterpret_cast<char *>(dst + q), src);
+        cp_async16(reinterpret_cast<char *>(dst + q) + 16, src + 16);
     }
 }
 
 // All the tiles of this block for one time step.  `n0` = number of tiles this block has pushed
 // through the pipeline before (persistent loop), which fixes the buffers and barrier parities.
 // Returns this thread's maximum rate contribution.
-__device__ __forceinline__ double step_tiles(const Params &P, const TilePipe &pp,
+template <int TC>
+__device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC> &pp,
                                              const Rec *__restrict__ Uin, Rec *__restrict__ Uout,
                                              const double dt, unsigned &nclamp, unsigned &n0)
 {
-    const int TC = blockDim.x, tid = threadIdx.x, G = gridDim.x;
+    const int tid = threadIdx.x, G = gridDim.x;
     double rate = 0.0;
     unsigned n = n0;
     int tile = blockIdx.x;
     if (tile >= P.ntiles) return 0.0;
-    // ---- prologue: everything tile n needs, and the halo ids of tile n+1
+    // ---- prologue: everything tile n needs, and the info block of tile n+1
     if (tid == 0) {
-        issue_halo_ids(P, pp, tile, n % 3);
+        issue_info(P, pp, tile, n % 3);
         issue_recs(P, pp, Uin, tile, n & 1);
-        issue_edges(P, pp, tile);
-        if (tile + G < P.ntiles) issue_halo_ids(P, pp, tile + G, (n + 1) % 3);
+        const int32_t *gi = P.tinfo + (size_t)tile * pp.info_stride;
+        issue_edges(P, pp, __ldg(gi), __ldg(gi + 1));
+        if (tile + G < P.ntiles) issue_info(P, pp, tile + G, (n + 1) % 3);
     }
-    mbar_wait(pp.hbar(n % 3), (n / 3) & 1u);
-    gather_halo(P, pp, Uin, tile, n % 3, n & 1);
+    mbar_wait(pp.ibar(n % 3), (n / 3) & 1u);
+    gather_halo(pp, Uin, n % 3, n & 1);
     cp_async_commit();
+    double *const so = pp.so;
+    const EdgeRec *const sedge = pp.sedge;
     for (; tile < P.ntiles; tile += G, n++) {
         const int s = n & 1;
         const int base = tile * TC;
-        const int ne = __ldg(P.estart + tile + 1) - __ldg(P.estart + tile);
         const bool have_next = tile + G < P.ntiles;
         // ---- top
         cp_async_wait<0>();                               // own halo gathers of this tile
@@ -472,7 +470,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe &pp
         __syncthreads();     // everyone has left the previous tile; everyone's gathers are visible
         if (tid == 0 && have_next) {
             issue_recs(P, pp, Uin, tile + G, s ^ 1);
-            if (tile + 2 * G < P.ntiles) issue_halo_ids(P, pp, tile + 2 * G, (n + 2) % 3);
+            if (tile + 2 * G < P.ntiles) issue_info(P, pp, tile + 2 * G, (n + 2) % 3);
         }
         if (base + tid < P.nt) {
             const double *src = P.cellc + (size_t)tile * 3 * TC + tid;
@@ -481,15 +479,15 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe &pp
         }
         cp_async_commit();
         if (have_next) {
-            mbar_wait(pp.hbar((n + 1) % 3), ((n + 1) / 3) & 1u);
-            gather_halo(P, pp, Uin, tile + G, (n + 1) % 3, s ^ 1);
+            mbar_wait(pp.ibar((n + 1) % 3), ((n + 1) / 3) & 1u);
+            gather_halo(pp, Uin, (n + 1) % 3, s ^ 1);
         }
         cp_async_commit();
-        const Rec *srec = pp.srec(s);
-        double *so = pp.so;
+        const Rec *const srec = pp.srec(s);
+        const int ne = pp.sinfo(n % 3)[1];
         // ---- phase 1: every edge of the tile once, shared memory only
         for (int e = tid; e < ne; e += TC) {
-            const EdgeRec er = pp.sedge[e];
+            const EdgeRec er = sedge[e];
             const int ia = er.a & kIdMask, ka = er.a >> kIdBits;
             const Rec A = srec[ia];
             Rec B;
@@ -498,17 +496,20 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe &pp
             double o[5];
             edge_eval(P, er, A, B, o);
             if (ia < TC) {
-                double *q = so + (ka * 3) * TC + ia;
+                double *q = so + ka * (3 * TC) + ia;
                 q[0] = o[0]; q[TC] = o[1]; q[2 * TC] = o[2];
             }
             if (ib < TC) {
-                double *q = so + (kb * 3) * TC + ib;
+                double *q = so + kb * (3 * TC) + ib;
                 q[0] = -o[0]; q[TC] = -o[3]; q[2 * TC] = -o[4];
             }
         }
         cp_async_wait<1>();                               // this tile's cell constants
         __syncthreads();
-        if (tid == 0 && have_next) issue_edges(P, pp, tile + G);
+        if (tid == 0 && have_next) {
+            const int32_t *ni = pp.sinfo((n + 1) % 3);
+            issue_edges(P, pp, ni[0], ni[1]);
+        }
         // ---- phase 2: every cell of the tile
         const int i = base + tid;
         if (i < P.nt) {

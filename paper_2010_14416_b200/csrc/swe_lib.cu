@@ -19,7 +19,7 @@ using namespace swe;
 // =================================================================================================
 namespace {
 
-constexpr int kDefaultBlock = 256;   // cells per tile = threads per block
+constexpr int kDefaultBlock = 192;   // cells per tile = threads per block (best of 128/192/256 on B200)
 constexpr int kMaxBlock = 256;
 #ifndef SWE_MIN_BLOCKS
 #define SWE_MIN_BLOCKS 3
@@ -27,35 +27,30 @@ constexpr int kMaxBlock = 256;
 constexpr int kMaxPart = 8192;       // upper bound on the grid of the step kernel
 extern __shared__ __align__(32) unsigned char dyn_smem[];
 
-__device__ __forceinline__ TilePipe pipe_setup(const Params &P)
+// nsteps time steps.  Every block first reduces the per-block maxima of the previous step into
+// dt (redundantly: a few KB from L2), so no separate finaliser launch and no atomics sit between
+// two steps; block 0 advances the device clock.  Blocks walk the tiles with a stride of the grid
+// through the TMA pipeline of swe_kernels.cuh.  TC = cells per tile = threads per block.
+//   graph / launch mode: nsteps = 1 per launch, the kernel boundary separates the steps;
+//   persistent mode: one cooperative launch runs the whole loop with a grid barrier between
+//   steps (PAPER.md:517: small meshes are "strictly limited by latencies" of kernel launches).
+// One kernel serves all modes, so their results are bitwise identical by construction.
+template <int TC>
+__global__ void __launch_bounds__(TC, (SWE_MIN_BLOCKS * kMaxBlock) / TC)
+swe_step_kernel(const Params P, int cur, const long long nsteps)
 {
-    const TilePipe pp = make_pipe(P, dyn_smem);
+    __shared__ double s_red[32];
+    const TilePipe<TC> pp = make_pipe<TC>(P, dyn_smem);
     if (threadIdx.x == 0) {
         for (int s = 0; s < kNumBars; s++) mbar_init(pp.bar + s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    return pp;
-}
-
-// nsteps time steps.  Every block first reduces the per-block maxima of the previous step into
-// dt (redundantly: a few KB from L2), so no separate finaliser launch and no atomics sit between
-// two steps; block 0 advances the device clock.  Blocks walk the tiles with a stride of the grid
-// through the two-stage TMA pipeline of swe_kernels.cuh.
-//   graph / launch mode: nsteps = 1 per launch, the kernel boundary separates the steps;
-//   persistent mode: one cooperative launch runs the whole loop with a grid barrier between
-//   steps (PAPER.md:517: small meshes are "strictly limited by latencies" of kernel launches).
-// One kernel serves all modes, so their results are bitwise identical by construction.
-__global__ void __launch_bounds__(kMaxBlock, SWE_MIN_BLOCKS)
-swe_step_kernel(const Params P, int cur, const long long nsteps)
-{
-    __shared__ double s_red[32];
-    const TilePipe pp = pipe_setup(P);
     unsigned it = 0;
     for (long long s = 0; s < nsteps; s++) {
         const double dt = reduce_dt(P, P.pmax(cur), s_red);
         unsigned nclamp = 0;
-        double rate = step_tiles(P, pp, P.U(cur), P.U(cur ^ 1), dt, nclamp, it);
+        double rate = step_tiles<TC>(P, pp, P.U(cur), P.U(cur ^ 1), dt, nclamp, it);
         rate = block_max(rate, s_red);
         if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
         if (threadIdx.x == 0) {
@@ -72,6 +67,18 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
             asm volatile("fence.proxy.async;" ::: "memory");
             cg::this_grid().sync();
         }
+    }
+}
+
+typedef void (*step_kernel_t)(const Params, int, const long long);
+step_kernel_t step_kernel_for(int tc)
+{
+    switch (tc) {
+    case 64: return swe_step_kernel<64>;
+    case 128: return swe_step_kernel<128>;
+    case 192: return swe_step_kernel<192>;
+    case 256: return swe_step_kernel<256>;
+    default: return nullptr;
     }
 }
 
@@ -144,7 +151,8 @@ struct swe_mesh {
     int32_t *d_perm = nullptr; double *d_zcell = nullptr; double *d_stage = nullptr;
     double *d_qn = nullptr;
     int cur = 0, grid = 0, block = kDefaultBlock, coop_grid = 0, loop_mode = SWE_LOOP_LAUNCH;
-    size_t smem = 0;          // dynamic shared memory of the step kernels
+    size_t smem = 0;          // dynamic shared memory of the step kernel
+    void (*kern)(const Params, int, const long long) = nullptr;
     int64_t launches = 0;
     double qn_tag[SWE_BC_MAX_TAG + 1] = {};
     std::map<std::pair<int, int>, cudaGraphExec_t> graphs; // (steps, cur) -> exec
@@ -166,7 +174,7 @@ static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 namespace {
 static_assert(sizeof(HostEdge) == sizeof(EdgeRec) && kHostIdBits == kIdBits, "table records");
 struct Layout {
-    size_t U0, U1, cellc, edges, estart, halo, hstart, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
+    size_t U0, U1, cellc, edges, tinfo, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
 };
 Layout make_layout(const HostTables &T, const TileTables &X)
 {
@@ -174,8 +182,7 @@ Layout make_layout(const HostTables &T, const TileTables &X)
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     L.U0 = take(n * sizeof(Rec)); L.U1 = take(n * sizeof(Rec));
     L.cellc = take(X.cellc.size() * sizeof(double)); L.edges = take(X.edges.size() * sizeof(EdgeRec));
-    L.estart = take(X.estart.size() * sizeof(int32_t));
-    L.halo = take(X.halo.size() * sizeof(int32_t) + 16); L.hstart = take(X.hstart.size() * sizeof(int32_t));
+    L.tinfo = take(X.tinfo.size() * sizeof(int32_t));
     L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
     L.stage = take(3 * n * sizeof(double));
     L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
@@ -212,8 +219,8 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     if (params) p = *params;
     if (!(p.g > 0.0) || !(p.cfl > 0.0) || !(p.h_dry >= 0.0) || p.ordering < 0 || p.ordering > SWE_ORDER_RCM ||
         p.loop_mode < 0 || p.loop_mode > SWE_LOOP_LAUNCH ||
-        (p.block_size != 0 && (p.block_size < 64 || p.block_size > kMaxBlock || p.block_size % 32))) {
-        g_create_err = "swe_mesh_create: invalid swe_params (block_size must be a multiple of 32 in [64, 256])";
+        (p.block_size != 0 && p.block_size != 64 && p.block_size != 128 && p.block_size != 192 && p.block_size != 256)) {
+        g_create_err = "swe_mesh_create: invalid swe_params (block_size must be 0, 64, 128, 192 or 256)";
         return SWE_ERR_INVALID_ARG;
     }
     swe_mesh *m = new (std::nothrow) swe_mesh();
@@ -300,9 +307,10 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     const TileTables &X = m->X;
     m->smem = tile_smem_bytes(m->block, X.max_halo, X.max_edges);
     if (m->smem > (size_t)smem_optin) { m->err = "tile does not fit in shared memory"; return SWE_ERR_CUDA; }
-    CK(cudaFuncSetAttribute(swe_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem));
+    m->kern = step_kernel_for(m->block);
+    CK(cudaFuncSetAttribute((const void *)m->kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem));
     int occ_step = 0, occ_pers = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_step, swe_step_kernel, m->block, m->smem));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_step, (const void *)m->kern, m->block, m->smem));
     occ_pers = occ_step;
     if (occ_step < 1 || occ_pers < 1) { m->err = "kernel does not fit on this device"; return SWE_ERR_CUDA; }
     const int ntiles = (int)X.ntiles;
@@ -318,8 +326,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     Params &P = m->P;
     P.U0 = (Rec *)(m->ws + L.U0); P.U1 = (Rec *)(m->ws + L.U1);
     P.cellc = (const double *)(m->ws + L.cellc); P.edges = (const EdgeRec *)(m->ws + L.edges);
-    P.estart = (const int32_t *)(m->ws + L.estart);
-    P.halo = (const int32_t *)(m->ws + L.halo); P.hstart = (const int32_t *)(m->ws + L.hstart);
+    P.tinfo = (const int32_t *)(m->ws + L.tinfo);
     m->d_zcell = (double *)(m->ws + L.zcell); m->d_perm = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
@@ -327,7 +334,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.ctrl = (Ctrl *)(m->ws + L.ctrl);
     P.nt = (int32_t)T.nt; P.ntiles = ntiles; P.max_edges = X.max_edges; P.max_halo = X.max_halo;
     P.npart = mode == SWE_LOOP_PERSISTENT ? m->coop_grid : m->grid;
-    P.g = m->prm.g; P.inv_g = 1.0 / m->prm.g; P.cfl = m->prm.cfl;
+    P.g = m->prm.g; P.hg = 0.5 * m->prm.g; P.inv_g = 1.0 / m->prm.g; P.cfl = m->prm.cfl;
     // a side is dry iff h <= h_dry; the floor keeps every argument of the MUFU-seeded
     // reciprocal / rsqrt a normal number when the caller asks for h_dry = 0
     P.hdry = std::max(m->prm.h_dry, 1e-250);
@@ -338,9 +345,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
         cudaStream_t s = m->stream;
         CK(cudaMemcpyAsync(m->ws + L.cellc, X.cellc.data(), X.cellc.size() * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.edges, X.edges.data(), X.edges.size() * sizeof(EdgeRec), cudaMemcpyHostToDevice, s));
-        CK(cudaMemcpyAsync(m->ws + L.estart, X.estart.data(), X.estart.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
-        if (!X.halo.empty()) CK(cudaMemcpyAsync(m->ws + L.halo, X.halo.data(), X.halo.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
-        CK(cudaMemcpyAsync(m->ws + L.hstart, X.hstart.data(), X.hstart.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.tinfo, X.tinfo.data(), X.tinfo.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_zcell, zc.data(), n * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_perm, T.perm.data(), n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_qn, m->qn_tag, sizeof(m->qn_tag), cudaMemcpyHostToDevice, s));
@@ -449,7 +454,7 @@ int swe_compute_dt(swe_mesh *m, double *dt_out)
 static int launch_steps_direct(swe_mesh *m, int64_t n)
 {
     for (int64_t s = 0; s < n; s++) {
-        swe_step_kernel<<<m->grid, m->block, m->smem, m->stream>>>(m->P, m->cur, 1);
+        m->kern<<<m->grid, m->block, m->smem, m->stream>>>(m->P, m->cur, 1);
         m->cur ^= 1;
         m->launches++;
     }
@@ -469,7 +474,7 @@ static int graph_for(swe_mesh *m, int steps, cudaGraphExec_t *out)
     cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
     int c = m->cur;
     if (e == cudaSuccess) {
-        for (int s = 0; s < steps; s++) { swe_step_kernel<<<m->grid, m->block, m->smem, cap>>>(m->P, c, 1); c ^= 1; }
+        for (int s = 0; s < steps; s++) { m->kern<<<m->grid, m->block, m->smem, cap>>>(m->P, c, 1); c ^= 1; }
         e = cudaStreamEndCapture(cap, &g);
     }
     if (e == cudaSuccess) e = cudaGraphInstantiate(&ex, g, 0);
@@ -492,7 +497,7 @@ int swe_run(swe_mesh *m, int64_t nsteps)
     if (m->loop_mode == SWE_LOOP_PERSISTENT) {
         Params P = m->P; int cur = m->cur; long long ns = nsteps;
         void *args[] = { &P, &cur, &ns };
-        CK(cudaLaunchCooperativeKernel((void *)swe_step_kernel, dim3(m->coop_grid), dim3(m->block), args, m->smem, m->stream));
+        CK(cudaLaunchCooperativeKernel((void *)m->kern, dim3(m->coop_grid), dim3(m->block), args, m->smem, m->stream));
         m->launches++;
         m->cur ^= (int)(nsteps & 1);
         return SWE_OK;
