@@ -62,9 +62,10 @@ enum { SWE_LOOP_AUTO = 0, SWE_LOOP_GRAPH = 1, SWE_LOOP_PERSISTENT = 2, SWE_LOOP_
 typedef struct {
     double g;           /* gravitational acceleration; the paper gives no value, default 9.81 */
     double cfl;         /* CFL number of eq.(15); default 0.9 */
-    double h_dry;       /* wet/dry threshold: a cell or edge side is dry iff h <= h_dry; 1e-6 */
+    double h_dry;       /* wet/dry threshold: a cell or edge side is dry iff h <= h_dry; 1e-6.
+                           Values below 1e-250 act as 1e-250 (keeps every rsqrt argument normal) */
     int32_t ordering;   /* SWE_ORDER_*; default SWE_ORDER_HILBERT */
-    int32_t block_size; /* CUDA threads per block, multiple of 32 in [64, 1024]; 0 = default */
+    int32_t block_size; /* cells per tile = CUDA threads per block: 64, 128, 192 or 256; 0 = default (192) */
     int32_t loop_mode;  /* SWE_LOOP_*; default SWE_LOOP_AUTO */
     int32_t reserved;   /* must be 0 */
 } swe_params;
@@ -94,8 +95,8 @@ int swe_params_default(swe_params *p);
  *   bc_tags     host [nt][3]  boundary tag per local edge, read only where the edge has no
  *                             neighbour; <= 0 or missing means SWE_BC_WALL
  *   params      host          NULL = defaults
- * Tables built (SoA, in the internal cell order): neighbour index per edge, unit outward
- * normal, L_ij / |Omega_i|, 1 / R_i, g m^2, cell bed.  nt < 2^31.  No CUDA call is made.
+ * Tables built (in the internal cell order): per-tile edge lists (end points, unit normal, length),
+ * halo lists, 1 / |Omega_i|, 1 / R_i, g m^2, cell bed.  nt < 2^29.  No CUDA call is made.
  */
 int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_t nt,
                     const double *bathymetry, const double *manning, const int8_t *bc_tags,
@@ -171,6 +172,28 @@ int swe_get_permutation(const swe_mesh *mesh, int32_t *perm);
  */
 int swe_get_tables(const swe_mesh *mesh, int32_t *nbr, double *normal, double *length,
                    double *area, double *inradius, double *cell_z);
+
+/*
+ * Tile decomposition of the step kernel: the internal cell order is cut
+ * into tiles of tile_cells consecutive cells (= swe_params.block_size); every edge touching a
+ * tile is listed once in that tile (an edge between two tiles is listed in both, so
+ * nedges / nt >= 1.5 measures the locality of the ordering).  max_edges / max_halo: longest edge
+ * list / halo list of any tile; smem_bytes: dynamic shared memory per block.  Any pointer may be NULL.
+ */
+int swe_get_tile_info(const swe_mesh *mesh, int32_t *tile_cells, int64_t *ntiles, int64_t *nedges,
+                      int32_t *max_edges, int32_t *max_halo, size_t *smem_bytes);
+
+/*
+ * The tile tables themselves, for tests of the mesh builder; any pointer may be NULL.
+ *   edge_a, edge_b [nedges]   end points: bits 0-28 = position in the tile's record array (local
+ *                             cell index if < tile_cells, else tile_cells + index into the tile's
+ *                             halo list), bits 29-30 = local edge index in that cell; edge_b = -tag
+ *                             on a boundary edge; a is the end point with the smaller caller id
+ *   edge_geom [nedges][3]     a's unit outward normal (n1, n2) and the edge length
+ *   tinfo [ntiles][4+max_halo] {first edge, #edges, #halo ids, 0, halo ids (internal), -1 padding}
+ */
+int swe_get_tile_tables(const swe_mesh *mesh, int32_t *edge_a, int32_t *edge_b, double *edge_geom,
+                        int32_t *tinfo);
 
 /* Launch facts for reporting: grid, block, loop mode actually in use, kernel launches issued
  * by this handle so far (step, rate, pack/unpack kernels). */

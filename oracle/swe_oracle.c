@@ -21,9 +21,9 @@
  *                        G(U,U) = physical flux, supercritical upwinding, antisymmetry
  *   geometry/neighbours: 2-triangle hand-computed update, rotation invariance
  *   bathymetry source  : lake at rest over a variable bed incl. emergent cells
- *   friction           : closed form q/(1 + dt c |q|) for uniform flow; m = 0 identity.
- *                        The d/dh column of the Jacobian (eq. 35) is PARITY UNPINNED:
- *                        no closed form or invariant isolates it.
+ *   friction           : closed form q/(1 + dt c |q|) for uniform flow; m = 0 identity;
+ *                        the whole Jacobian incl. its d/dh column against the symbolic
+ *                        derivative of eq. (32) (its definition, eq. 34) on a non-uniform state
  *   whole step         : Stoker and Ritter dam-break solutions, mass conservation,
  *                        mirror symmetry
  *   dt                 : closed form CFL * R_min / (sqrt(g h) + |V|) on a uniform state

@@ -25,7 +25,8 @@ SYMBOLS = [
     "swe_params_default", "swe_mesh_create", "swe_mesh_destroy", "swe_mesh_workspace_bytes",
     "swe_mesh_bind_device", "swe_set_bc_value", "swe_set_state", "swe_set_state_device",
     "swe_compute_dt", "swe_step", "swe_run", "swe_sync", "swe_get_state", "swe_get_state_device",
-    "swe_get_stats", "swe_get_permutation", "swe_get_tables", "swe_get_launch_info",
+    "swe_get_stats", "swe_get_permutation", "swe_get_tables", "swe_get_tile_info",
+    "swe_get_tile_tables", "swe_get_launch_info",
     "swe_last_error",
 ]
 
@@ -79,6 +80,9 @@ def load_library(rebuild_if_stale: bool = True):
     L.swe_get_stats.argtypes = [vp, C.POINTER(SweStats)]
     L.swe_get_permutation.argtypes = [vp, i32p]
     L.swe_get_tables.argtypes = [vp, i32p, dp, dp, dp, dp, dp]
+    L.swe_get_tile_info.argtypes = [vp, i32p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), i32p, i32p,
+                                    C.POINTER(C.c_size_t)]
+    L.swe_get_tile_tables.argtypes = [vp, i32p, i32p, dp, i32p]
     L.swe_get_launch_info.argtypes = [vp, i32p, i32p, i32p, C.POINTER(C.c_int64)]
     L.swe_last_error.argtypes = [vp]
     L.swe_last_error.restype = C.c_char_p
@@ -236,6 +240,26 @@ class SweMesh:
         self._ck(self._L.swe_get_tables(self._h, nbr.ctypes.data_as(C.POINTER(C.c_int32)),
                                         _dp(normal), _dp(length), _dp(area), _dp(rin), _dp(z)))
         return dict(nbr=nbr, normal=normal, length=length, area=area, inradius=rin, cell_z=z)
+
+    def get_tile_info(self) -> dict:
+        tc, mx, mh = C.c_int32(0), C.c_int32(0), C.c_int32(0)
+        nti, ne, sm = C.c_int64(0), C.c_int64(0), C.c_size_t(0)
+        self._ck(self._L.swe_get_tile_info(self._h, C.byref(tc), C.byref(nti), C.byref(ne), C.byref(mx),
+                                           C.byref(mh), C.byref(sm)))
+        return dict(tile_cells=tc.value, ntiles=nti.value, nedges=ne.value, max_edges=mx.value,
+                    max_halo=mh.value, smem_bytes=sm.value, edges_per_cell=ne.value / self.nt)
+
+    def get_tile_tables(self) -> dict:
+        ti = self.get_tile_info()
+        ne, stride = ti["nedges"], 4 + ti["max_halo"]
+        a = np.empty(ne, dtype=np.int32)
+        b = np.empty(ne, dtype=np.int32)
+        geom = np.empty((ne, 3), dtype=np.float64)
+        tinfo = np.empty((ti["ntiles"], stride), dtype=np.int32)
+        i32p = C.POINTER(C.c_int32)
+        self._ck(self._L.swe_get_tile_tables(self._h, a.ctypes.data_as(i32p), b.ctypes.data_as(i32p),
+                                             _dp(geom), tinfo.ctypes.data_as(i32p)))
+        return dict(edge_a=a, edge_b=b, edge_geom=geom, tinfo=tinfo, **ti)
 
     def get_launch_info(self) -> dict:
         g, b, lm, n = C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int64(0)

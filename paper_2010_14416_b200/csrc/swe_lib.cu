@@ -83,7 +83,7 @@ step_kernel_t step_kernel_for(int tc)
 }
 
 // Per-block maxima of (sqrt(g h)+|V|)/R for the state in U[cur] (swe_compute_dt, first step).
-__global__ void __launch_bounds__(kDefaultBlock)
+__global__ void __launch_bounds__(kMaxBlock)
 swe_rate_kernel(const Params P, const int cur)
 {
     __shared__ double s_red[32];
@@ -271,6 +271,33 @@ int swe_get_tables(const swe_mesh *m, int32_t *nbr, double *normal, double *leng
     if (area) std::memcpy(area, m->T.area.data(), n * sizeof(double));
     if (inradius) std::memcpy(inradius, m->T.inradius.data(), n * sizeof(double));
     if (cell_z) std::memcpy(cell_z, m->T.cell_z.data(), n * sizeof(double));
+    return SWE_OK;
+}
+
+int swe_get_tile_info(const swe_mesh *m, int32_t *tile_cells, int64_t *ntiles, int64_t *nedges,
+                      int32_t *max_edges, int32_t *max_halo, size_t *smem_bytes)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    if (tile_cells) *tile_cells = m->X.tile_cells;
+    if (ntiles) *ntiles = m->X.ntiles;
+    if (nedges) *nedges = (int64_t)m->X.edges.size();
+    if (max_edges) *max_edges = m->X.max_edges;
+    if (max_halo) *max_halo = m->X.max_halo;
+    if (smem_bytes) *smem_bytes = tile_smem_bytes(m->X.tile_cells, m->X.max_halo, m->X.max_edges);
+    return SWE_OK;
+}
+
+int swe_get_tile_tables(const swe_mesh *m, int32_t *edge_a, int32_t *edge_b, double *edge_geom, int32_t *tinfo)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    const size_t ne = m->X.edges.size();
+    for (size_t e = 0; e < ne; e++) {
+        const HostEdge &E = m->X.edges[e];
+        if (edge_a) edge_a[e] = E.a;
+        if (edge_b) edge_b[e] = E.b;
+        if (edge_geom) { edge_geom[3 * e] = E.n1; edge_geom[3 * e + 1] = E.n2; edge_geom[3 * e + 2] = E.len; }
+    }
+    if (tinfo) std::memcpy(tinfo, m->X.tinfo.data(), m->X.tinfo.size() * sizeof(int32_t));
     return SWE_OK;
 }
 

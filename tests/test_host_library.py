@@ -128,3 +128,57 @@ def test_compute_entry_points_fail_loudly_without_a_device():
     with pytest.raises(B.SweError) as e:
         m.set_bc_value(3, 1.0)       # no edge carries tag 3 on this mesh
     assert e.value.code == -11
+
+
+@pytest.mark.parametrize("ordering", [B.ORDER_IDENTITY, B.ORDER_HILBERT, B.ORDER_RCM])
+@pytest.mark.parametrize("block", [64, 192, 256])
+def test_tile_tables_cover_every_cell_edge_exactly_once(ordering, block):
+    """Tile tables of the step kernel, checked against the ORACLE's neighbour/geometry tables:
+    every (cell, local edge) is the a- or b-side of exactly one edge record of its tile, that
+    record's other end is the oracle's neighbour (through the halo list if it lives in another
+    tile), a is the smaller caller id, the normal is a's outward normal and the tag matches."""
+    w = W.config4(nx=50, ny=13)              # ragged last tile, inflow / outflow / wall tags
+    m = B.SweMesh.from_workload(w, ordering=ordering, block_size=block)
+    X = m.get_tile_tables()
+    geo = OracleSolver.from_workload(w).geometry()
+    perm = m.get_permutation()
+    nt, TC = w.ncells, X["tile_cells"]
+    assert TC == block and X["ntiles"] == (nt + TC - 1) // TC
+    seen = np.zeros((nt, 3), dtype=np.int32)
+    mask = (1 << 29) - 1
+    assert X["tinfo"][:, 0].tolist() == np.concatenate([[0], np.cumsum(X["tinfo"][:, 1])[:-1]]).tolist()
+    assert X["tinfo"][:, 1].sum() == X["nedges"] and X["tinfo"][:, 1].max() == X["max_edges"]
+    for t in range(X["ntiles"]):
+        e0, ne, nh = X["tinfo"][t, :3]
+        halo = X["tinfo"][t, 4:4 + nh]
+        assert nh <= X["max_halo"] and len(set(halo.tolist())) == nh
+        assert ((halo < t * TC) | (halo >= (t + 1) * TC)).all()      # halo cells live in other tiles
+        assert (X["tinfo"][t, 4 + nh:] == -1).all()
+
+        def internal(pos):
+            return t * TC + pos if pos < TC else halo[pos - TC]
+
+        for e in range(e0, e0 + ne):
+            a, b = int(X["edge_a"][e]), int(X["edge_b"][e])
+            pa, ka = internal(a & mask), a >> 29
+            ca = perm[pa]
+            n1, n2, L = X["edge_geom"][e]
+            assert abs(n1 - geo["n1"][ca, ka]) <= 1e-15 and abs(n2 - geo["n2"][ca, ka]) <= 1e-15
+            assert L == pytest.approx(geo["len"][ca, ka], rel=1e-15)
+            if (a & mask) < TC:
+                seen[ca, ka] += 1
+            if b < 0:                                                  # boundary edge
+                assert geo["nbr"][ca, ka] < 0 and -b == max(int(w.bc_tags[ca, ka]), 1)
+                assert (a & mask) < TC
+                continue
+            pb, kb = internal(b & mask), b >> 29
+            cb = perm[pb]
+            assert geo["nbr"][ca, ka] == cb and geo["nbr"][cb, kb] == ca and ca < cb
+            assert (a & mask) < TC or (b & mask) < TC                  # the edge touches this tile
+            if (b & mask) < TC:
+                seen[cb, kb] += 1
+    assert (seen == 1).all()
+    # locality: a space-filling-curve order keeps most edges inside one tile
+    if ordering == B.ORDER_HILBERT and block >= 192:
+        assert X["edges_per_cell"] < 1.85
+    assert 1.5 <= X["edges_per_cell"] <= 3.0

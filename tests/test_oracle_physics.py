@@ -215,3 +215,46 @@ def test_ritter_front_and_profile():
         assert np.abs(h[cx < 50.0 - 1.05 * math.sqrt(G) * t - 2.0] - 1.0).max() < 0.01
     assert errs[1] < 0.75 * errs[0]
     assert tips[1] > tips[0]
+
+
+def test_friction_jacobian_including_h_column_vs_symbolic_derivative():
+    """eq.(34)-(37), R-19: J_f is DEFINED as dS_f/dU of eq.(32).  The oracle's step must satisfy
+    [I - dt/2 J] dU = dt (b + S_f) with J taken here by symbolic differentiation of eq.(32)
+    (sympy), not from the printed matrix (35).  dt*b comes from the same step without friction.
+    The d/dh column matters: the same residual with that column zeroed is orders larger."""
+    import sympy as sp
+    h, qx, qy, gg, mm = sp.symbols("h qx qy g m", positive=True)
+    qn = sp.sqrt(qx ** 2 + qy ** 2)
+    Sf = sp.Matrix([0, -gg * mm ** 2 * qx * qn / h ** sp.Rational(7, 3),
+                    -gg * mm ** 2 * qy * qn / h ** sp.Rational(7, 3)])          # eq.(32), PAPER.md:227
+    Jf = Sf.jacobian([h, qx, qy])
+    f_S = sp.lambdify((h, qx, qy, gg, mm), Sf, "numpy")
+    f_J = sp.lambdify((h, qx, qy, gg, mm), Jf, "numpy")
+
+    mn = 0.04
+    w0 = W.canal_dam_break(30, 4, h_left=1.3, h_right=0.4, manning=0.0, length=30.0, seed=11)
+    rng = np.random.default_rng(5)
+    w0.hu[:] = w0.h * rng.uniform(0.5, 2.0, w0.ncells)
+    w0.hv[:] = w0.h * rng.uniform(-1.0, 1.0, w0.ncells)
+    w1 = W.canal_dam_break(30, 4, h_left=1.3, h_right=0.4, manning=mn, length=30.0, seed=11)
+    w1.hu[:], w1.hv[:] = w0.hu, w0.hv
+    dt = 0.05
+    a, b = OracleSolver.from_workload(w0), OracleSolver.from_workload(w1)
+    a.step_dt(dt)
+    b.step_dt(dt)
+    U = np.stack([w0.h, w0.hu, w0.hv], 1)
+    dU0 = np.stack(a.get_state()[:3], 1) - U            # dt * b
+    dU1 = np.stack(b.get_state()[:3], 1) - U
+    assert np.abs(dU0[:, 0]).max() > 1e-3                # depth does change: the h column is exercised
+    worst, worst_noh = 0.0, 0.0
+    for i in range(w0.ncells):
+        S = np.array(f_S(U[i, 0], U[i, 1], U[i, 2], G, mn), dtype=float).ravel()
+        J = np.array(f_J(U[i, 0], U[i, 1], U[i, 2], G, mn), dtype=float)
+        scale = np.abs(dU0[i]).max() + dt * np.abs(S).max()
+        r = (np.eye(3) - 0.5 * dt * J) @ dU1[i] - dU0[i] - dt * S
+        worst = max(worst, np.abs(r).max() / scale)
+        J[:, 0] = 0.0
+        r = (np.eye(3) - 0.5 * dt * J) @ dU1[i] - dU0[i] - dt * S
+        worst_noh = max(worst_noh, np.abs(r).max() / scale)
+    assert worst < 1e-12
+    assert worst_noh > 1e4 * max(worst, 1e-16)
