@@ -189,3 +189,65 @@ def test_device_state_roundtrip():
     np.testing.assert_array_equal(out[0].cpu().numpy(), h)
     np.testing.assert_array_equal(out[1].cpu().numpy(), hu)
     np.testing.assert_array_equal(out[2].cpu().numpy(), hv)
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times (defaults) ----------
+def test_config3_full_size_every_cell_then_invariants():
+    """configs[2] at 2000x1000 squares (4,000,000 cells): every cell against the oracle after 40
+    steps, then the remaining steps of the 1000 on the GPU alone, checked by what holds at any
+    size: state at rest to round-off, dry mask unchanged, mass to round-off, dt constant."""
+    w = W.config3()
+    m, o = run_both(w, 40)
+    assert_parity(m, o, w)
+    info = m.get_launch_info()
+    assert info["loop_mode"] == "graph" and info["block"] == 192
+    dt40 = m.get_state()[4]
+    m.run(w.nsteps - 40)
+    h, hu, hv, t, dt = m.get_state()
+    st = m.get_stats()
+    assert st["steps"] == w.nsteps and st["n_clamped"] == 0 and st["n_nonfinite"] == 0
+    tab = m.get_tables()
+    wet = h > w.h_dry
+    np.testing.assert_array_equal(~wet, w.h <= w.h_dry)
+    assert np.abs(h[wet] + tab["cell_z"][wet] - 2.0).max() < 1e-12
+    assert np.abs(hu[wet] / h[wet]).max() < 1e-10 and np.abs(hv[wet] / h[wet]).max() < 1e-10
+    assert st["volume"] == pytest.approx(float(np.sum(w.h * tab["area"])), rel=1e-12)
+    assert dt == pytest.approx(dt40, rel=1e-12)
+
+
+def test_config4_full_size_every_cell_then_mass_balance():
+    """configs[3] at 5100x1275 squares (13,005,000 cells): every cell against the oracle after 25
+    steps; then 2000 steps in all on the GPU: no clamp, nothing non-finite, and the volume gained
+    is the prescribed inflow (exactly, while the outlet is dry) minus what left through the outlet."""
+    w = W.config4()
+    m, o = run_both(w, 25)
+    assert_parity(m, o, w)
+    assert m.get_launch_info()["loop_mode"] == "graph"
+    v0 = float(np.sum(w.h * m.get_tables()["area"]))
+    m.run(w.nsteps - 25)
+    st = m.get_stats()
+    assert st["steps"] == w.nsteps and st["n_clamped"] == 0 and st["n_nonfinite"] == 0
+    h, hu, hv, t, dt = m.get_state()
+    assert h.min() >= 0.0 and dt > 0.0
+    cx = W.centroids(w.nodes_xy, w.tris)[:, 0]
+    outlet_wet = (cx > 0.999 * w.nodes_xy[:, 0].max()) & (h > w.h_dry) & (hu > 0)
+    gained = st["volume"] - v0
+    if not outlet_wet.any():
+        assert gained == pytest.approx(500.0 * t, rel=1e-9)     # R-20: all of Q enters, nothing leaves
+    else:                       # the outlet only removes water: the gain cannot exceed the inflow
+        assert gained <= 500.0 * t * (1 + 1e-9)
+
+
+def test_random_caller_numbering_without_locality_pass():
+    """config 5's 'random permutation' arm: ORDER_IDENTITY keeps the caller's random numbering,
+    so every neighbour lives in another tile (3 edge evaluations per cell, halo = 3 x tile)."""
+    w = W.config5("0.1M", nsteps=200)
+    m, o = run_both(w, 200, ordering=B.ORDER_IDENTITY)
+    assert_parity(m, o, w)
+    ti = m.get_tile_info()
+    assert ti["edges_per_cell"] > 2.9
+    m2 = B.SweMesh.from_workload(w, ordering=B.ORDER_HILBERT).bind_device()
+    m2.set_state(w.h, w.hu, w.hv)
+    m2.run(200)
+    for a, b in zip(m.get_state()[:3], m2.get_state()[:3]):
+        np.testing.assert_array_equal(a, b)                        # R-17, bitwise
