@@ -165,6 +165,21 @@ def run_reference(args, rank: int, world: int):
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks(values, world: int, device="cpu"):
+    """Element-wise max of a list of floats over all ranks (the job time is the slowest rank's)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def job_throughput(cells_per_rank: int, steps: int, world: int, ms_max: float) -> float:
+    """Replicas only: every rank steps its own copy; units of all ranks / slowest rank's time."""
+    return float(cells_per_rank) * steps * world / (ms_max * 1e-3)
+
+
 def run_gpu(args, rank: int, world: int, local_rank: int):
     import torch
     import torch.distributed as dist
@@ -231,17 +246,14 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - e0
 
-    times = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    ms, e2e_ms = times.tolist()
+    ms, e2e_ms = max_over_ranks([ms, e2e_s * 1e3], world, dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
     total_updates = float(n) * args.steps * world
-    value = total_updates / (ms * 1e-3)
+    value = job_throughput(n, args.steps, world, ms)
     peak, peak_src = load_peaks()
     kernel_ms = ms / args.steps                       # one step kernel launch per step
     achieved = ALGO_BYTES_PER_CELL * n / (kernel_ms * 1e-3) / 1e9
