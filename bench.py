@@ -257,6 +257,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     peak, peak_src = load_peaks()
     kernel_ms = ms / args.steps                       # one step kernel launch per step
     achieved = ALGO_BYTES_PER_CELL * n / (kernel_ms * 1e-3) / 1e9
+    traffic = load_traffic(args.workload)     # ncu dram bytes per launch of this workload (profiles/)
     sample, what = make_sample(args.workload)
     cpu_value, cpu_threads, _ = time_oracle(sample, 10 if sample.ncells > 300000 else 100, 2)
     line = {
@@ -274,7 +275,9 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                    "mesh_build_s": round(t_build, 2), "wet_fraction_end": 1.0 - stats["n_dry"] / n,
                    "n_clamped": stats["n_clamped"]},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": load_traffic(args.workload),
+                     "frac": achieved / peak, "traffic": traffic,
+                     "achieved_dram": None if traffic is None else traffic / (kernel_ms * 1e-3) / 1e9,
+                     "frac_dram": None if traffic is None else traffic / (kernel_ms * 1e-3) / 1e9 / peak,
                      "kernel": f"swe_step_kernel<{tiles['tile_cells']}>", "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
                      "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
         "cpu_baseline": {"value": cpu_value, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",

@@ -289,6 +289,8 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
             const int32_t nh = hstart[(size_t)t + 1] - hstart[(size_t)t];
             ti[0] = X.estart[(size_t)t]; ti[1] = X.estart[(size_t)t + 1] - X.estart[(size_t)t];
             ti[2] = nh; ti[3] = 0;
+            for (int32_t e = X.estart[(size_t)t]; e < X.estart[(size_t)t + 1]; e++)
+                if (X.edges[(size_t)e].b <= -SWE_BC_INFLOW0) ti[3] = 1;      // prescribed-discharge edge
             std::copy(halo.begin() + hstart[(size_t)t], halo.begin() + hstart[(size_t)t + 1], ti + 4);
         }
     } catch (const std::bad_alloc &) { err = "out of host memory"; return SWE_ERR_NOMEM; }

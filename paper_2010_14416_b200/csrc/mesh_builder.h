@@ -39,8 +39,8 @@ struct TileTables {
     int64_t ntiles = 0;
     int32_t max_edges = 0;             // longest edge list of any tile
     int32_t max_halo = 0;              // longest halo list of any tile, rounded up to a multiple of 4
-    // [ntiles][4 + max_halo]: {first edge, #edges, #halo ids, 0, halo ids (internal cell ids of the
-    // tile's off-tile end points) padded with -1}
+    // [ntiles][4 + max_halo]: {first edge, #edges, #halo ids, 1 if the tile has an inflow edge else 0,
+    // halo ids (internal cell ids of the tile's off-tile end points) padded with -1}
     std::vector<int32_t> tinfo;
     std::vector<int32_t> estart;       // [ntiles + 1] offsets into edges
     std::vector<HostEdge> edges;

@@ -352,7 +352,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 // ---- the tile pipeline -----------------------------------------------------------------------------
 // Per-tile info block in global memory (P.tinfo, fixed stride 4 + MH int32, MH = P.max_halo):
 //   [0] first edge of the tile in P.edges   [1] number of edges   [2] number of halo ids
-//   [3] reserved                            [4..] halo ids (internal cell ids), padded with -1
+//   [3] 1 if an inflow edge touches it      [4..] halo ids (internal cell ids), padded with -1
 // Shared memory of one block (dynamic); TC = blockDim.x, ME = P.max_edges:
 //   double  so[9][TC]              (local edge k, component) flux slots of the tile's cells
 //   Rec     srec[2][TC + MH]       state records of the tile's cells, then of its halo cells
@@ -467,12 +467,23 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
         cp_async_wait<0>();                               // own halo gathers of this tile
         mbar_wait(pp.rbar(s), (n >> 1) & 1u);
         mbar_wait(pp.ebar(), n & 1u);
-        __syncthreads();     // everyone has left the previous tile; everyone's gathers are visible
+        const Rec *const srec = pp.srec(s);
+        const int32_t *const info = pp.sinfo(n % 3);
+        const int ne = info[1], nh = info[2];
+        // is anything wet in the tile or its halo?  Each thread looks at its own record and at
+        // the halo records it gathered itself, so the vote can BE the tile's first barrier.
+        const int i = base + tid;
+        bool wet = i < P.nt && srec[tid].h > P.hdry;
+        if (!wet)       // a wet own cell already decides the vote
+            for (int q = tid; q < nh; q += TC) wet |= srec[TC + q].h > P.hdry;
+        // barrier: everyone has left the previous tile; everyone's gathers are visible
+        // (the warp vote only tells the compiler that the outcome is warp-uniform)
+        const bool active = __any_sync(0xffffffffu, __syncthreads_or(wet) || info[3] != 0);
         if (tid == 0 && have_next) {
             issue_recs(P, pp, Uin, tile + G, s ^ 1);
             if (tile + 2 * G < P.ntiles) issue_info(P, pp, tile + 2 * G, (n + 2) % 3);
         }
-        if (base + tid < P.nt) {
+        if (active && i < P.nt) {
             const double *src = P.cellc + (size_t)tile * 3 * TC + tid;
             double *dst = pp.scell + tid;
             cp_async8(dst, src); cp_async8(dst + TC, src + TC); cp_async8(dst + 2 * TC, src + 2 * TC);
@@ -483,46 +494,54 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
             gather_halo(pp, Uin, (n + 1) % 3, s ^ 1);
         }
         cp_async_commit();
-        const Rec *const srec = pp.srec(s);
-        const int ne = pp.sinfo(n % 3)[1];
-        // ---- phase 1: every edge of the tile once, shared memory only
-        for (int e = tid; e < ne; e += TC) {
-            const EdgeRec er = sedge[e];
-            const int ia = er.a & kIdMask, ka = er.a >> kIdBits;
-            const Rec A = srec[ia];
-            Rec B;
-            int ib = TC, kb = 0;
-            if (er.b >= 0) { ib = er.b & kIdMask; kb = er.b >> kIdBits; B = srec[ib]; }
-            double o[5];
-            edge_eval(P, er, A, B, o);
-            if (ia < TC) {
-                double *q = so + ka * (3 * TC) + ia;
-                q[0] = o[0]; q[TC] = o[1]; q[2 * TC] = o[2];
+        if (!active) {
+            // Every cell of the tile and every neighbour is dry and no discharge is prescribed:
+            // all fluxes vanish, h' = h + 0, and dry cells carry u = v = 0 already (R-15), so the
+            // step leaves the records unchanged bit for bit.  The copy still moves them.
+            if (tid == 0 && have_next) {
+                const int32_t *ni = pp.sinfo((n + 1) % 3);
+                issue_edges(P, pp, ni[0], ni[1]);
             }
-            if (ib < TC) {
-                double *q = so + kb * (3 * TC) + ib;
-                q[0] = -o[0]; q[TC] = -o[3]; q[2 * TC] = -o[4];
+            if (i < P.nt) store_rec(Uout + i, srec[tid]);
+        } else {
+            // ---- phase 1: every edge of the tile once, shared memory only
+            for (int e = tid; e < ne; e += TC) {
+                const EdgeRec er = sedge[e];
+                const int ia = er.a & kIdMask, ka = er.a >> kIdBits;
+                const Rec A = srec[ia];
+                Rec B;
+                int ib = TC, kb = 0;
+                if (er.b >= 0) { ib = er.b & kIdMask; kb = er.b >> kIdBits; B = srec[ib]; }
+                double o[5];
+                edge_eval(P, er, A, B, o);
+                if (ia < TC) {
+                    double *q = so + ka * (3 * TC) + ia;
+                    q[0] = o[0]; q[TC] = o[1]; q[2 * TC] = o[2];
+                }
+                if (ib < TC) {
+                    double *q = so + kb * (3 * TC) + ib;
+                    q[0] = -o[0]; q[TC] = -o[3]; q[2 * TC] = -o[4];
+                }
             }
-        }
-        cp_async_wait<1>();                               // this tile's cell constants
-        __syncthreads();
-        if (tid == 0 && have_next) {
-            const int32_t *ni = pp.sinfo((n + 1) % 3);
-            issue_edges(P, pp, ni[0], ni[1]);
-        }
-        // ---- phase 2: every cell of the tile
-        const int i = base + tid;
-        if (i < P.nt) {
-            const Rec Ui = srec[tid];
-            const double *sc = pp.scell + tid;
-            const double *q = so + tid;
-            // three edges in the fixed order k = 0,1,2 (R-17)
-            const double s1 = (q[0] + q[3 * TC]) + q[6 * TC];
-            const double s2 = (q[TC] + q[4 * TC]) + q[7 * TC];
-            const double s3 = (q[2 * TC] + q[5 * TC]) + q[8 * TC];
-            Rec Un;
-            rate = fmax(rate, cell_update(P, Ui, s1, s2, s3, sc[0], sc[TC], sc[2 * TC], dt, Un, nclamp));
-            store_rec(Uout + i, Un);
+            cp_async_wait<1>();                               // this tile's cell constants
+            __syncthreads();
+            if (tid == 0 && have_next) {
+                const int32_t *ni = pp.sinfo((n + 1) % 3);
+                issue_edges(P, pp, ni[0], ni[1]);
+            }
+            // ---- phase 2: every cell of the tile
+            if (i < P.nt) {
+                const Rec Ui = srec[tid];
+                const double *sc = pp.scell + tid;
+                const double *q = so + tid;
+                // three edges in the fixed order k = 0,1,2 (R-17)
+                const double s1 = (q[0] + q[3 * TC]) + q[6 * TC];
+                const double s2 = (q[TC] + q[4 * TC]) + q[7 * TC];
+                const double s3 = (q[2 * TC] + q[5 * TC]) + q[8 * TC];
+                Rec Un;
+                rate = fmax(rate, cell_update(P, Ui, s1, s2, s3, sc[0], sc[TC], sc[2 * TC], dt, Un, nclamp));
+                store_rec(Uout + i, Un);
+            }
         }
     }
     cp_async_wait<0>();
