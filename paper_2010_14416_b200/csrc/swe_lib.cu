@@ -110,24 +110,24 @@ __global__ void swe_finalize_dt_kernel(const Params P, const int cur)
 }
 
 // caller numbering (h, hu, hv) -> internal records {h, u, v, z}; dry cells lose their momentum
-__global__ void swe_pack_kernel(const Params P, const int cur, const int32_t *__restrict__ perm,
+// Both kernels run over the CALLER's numbering c (coalesced on the caller's arrays) and touch the
+// internal record inv[c] as one 32-byte sector.  zcell is in caller numbering too.
+__global__ void swe_pack_kernel(const Params P, const int cur, const int32_t *__restrict__ inv,
                                 const double *__restrict__ h, const double *__restrict__ hu,
                                 const double *__restrict__ hv, const double *__restrict__ zcell)
 {
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= P.nt) return;
-    const int c = perm[p];
-    Rec r; r.h = h[c]; r.z = zcell[p];
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.nt) return;
+    Rec r; r.h = h[c]; r.z = zcell[c];
     if (r.h > P.hdry) { r.u = hu[c] / r.h; r.v = hv[c] / r.h; } else { r.u = 0.0; r.v = 0.0; }
-    store_rec(P.U(cur) + p, r);
+    store_rec(P.U(cur) + inv[c], r);
 }
-__global__ void swe_unpack_kernel(const Params P, const int cur, const int32_t *__restrict__ perm,
+__global__ void swe_unpack_kernel(const Params P, const int cur, const int32_t *__restrict__ inv,
                                   double *__restrict__ h, double *__restrict__ hu, double *__restrict__ hv)
 {
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= P.nt) return;
-    const int c = perm[p];
-    const Rec r = load_rec(P.U(cur) + p);
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.nt) return;
+    const Rec r = load_rec(P.U(cur) + inv[c]);
     if (h) h[c] = r.h;
     if (hu) hu[c] = r.h * r.u;
     if (hv) hv[c] = r.h * r.v;
@@ -148,7 +148,7 @@ struct swe_mesh {
     char *ws = nullptr; size_t ws_bytes = 0;
     cudaStream_t stream = nullptr;
     Params P{};
-    int32_t *d_perm = nullptr; double *d_zcell = nullptr; double *d_stage = nullptr;
+    int32_t *d_inv = nullptr; double *d_zcell = nullptr; double *d_stage = nullptr;
     double *d_qn = nullptr;
     int cur = 0, grid = 0, block = kDefaultBlock, coop_grid = 0, loop_mode = SWE_LOOP_LAUNCH;
     size_t smem = 0;          // dynamic shared memory of the step kernel
@@ -354,7 +354,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.U0 = (Rec *)(m->ws + L.U0); P.U1 = (Rec *)(m->ws + L.U1);
     P.cellc = (const double *)(m->ws + L.cellc); P.edges = (const EdgeRec *)(m->ws + L.edges);
     P.tinfo = (const int32_t *)(m->ws + L.tinfo);
-    m->d_zcell = (double *)(m->ws + L.zcell); m->d_perm = (int32_t *)(m->ws + L.perm);
+    m->d_zcell = (double *)(m->ws + L.zcell); m->d_inv = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
     m->d_qn = (double *)(m->ws + L.qn); P.qn_tag = m->d_qn;
@@ -367,14 +367,12 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.hdry = std::max(m->prm.h_dry, 1e-250);
 
     try {
-        std::vector<double> zc(n);
-        for (size_t p = 0; p < n; p++) zc[p] = T.cell_z[(size_t)T.perm[p]];
         cudaStream_t s = m->stream;
         CK(cudaMemcpyAsync(m->ws + L.cellc, X.cellc.data(), X.cellc.size() * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.edges, X.edges.data(), X.edges.size() * sizeof(EdgeRec), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.tinfo, X.tinfo.data(), X.tinfo.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
-        CK(cudaMemcpyAsync(m->d_zcell, zc.data(), n * sizeof(double), cudaMemcpyHostToDevice, s));
-        CK(cudaMemcpyAsync(m->d_perm, T.perm.data(), n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->d_zcell, T.cell_z.data(), n * sizeof(double), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->d_inv, T.inv.data(), n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_qn, m->qn_tag, sizeof(m->qn_tag), cudaMemcpyHostToDevice, s));
         CK(cudaMemsetAsync(P.pmax0, 0, kMaxPart * sizeof(double), s));
         CK(cudaMemsetAsync(P.pmax1, 0, kMaxPart * sizeof(double), s));
@@ -405,7 +403,7 @@ static int set_state_common(swe_mesh *m, const double *h, const double *hu, cons
 {
     const int n = (int)m->T.nt;
     m->cur = 0;
-    swe_pack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_perm, h, hu, hv, m->d_zcell);
+    swe_pack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_inv, h, hu, hv, m->d_zcell);
     m->launches++;
     CK(cudaGetLastError());
     Ctrl c{}; c.t = t0;
@@ -562,7 +560,7 @@ int swe_get_state_device(swe_mesh *m, double *d_h, double *d_hu, double *d_hv)
     if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
     if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
     const int n = (int)m->T.nt;
-    swe_unpack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, m->cur, m->d_perm, d_h, d_hu, d_hv);
+    swe_unpack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, m->cur, m->d_inv, d_h, d_hu, d_hv);
     m->launches++;
     CK(cudaGetLastError());
     return SWE_OK;
