@@ -149,6 +149,25 @@ int swe_step(swe_mesh *mesh);
  */
 int swe_run(swe_mesh *mesh, int64_t nsteps);
 
+/*
+ * Steps until the simulated time reaches t_end (the paper specifies its runs by simulated time,
+ * PAPER.md:541, :611): the step that would pass t_end is shortened to end on it.  At most
+ * max_steps steps.  *steps_done (may be NULL) = steps actually taken.  Synchronises the stream
+ * (the host looks at the device clock between batches of steps; the steps themselves never leave
+ * the device).  Stops early if the domain becomes all dry.
+ */
+int swe_run_until(swe_mesh *mesh, double t_end, int64_t max_steps, int64_t *steps_done);
+
+/*
+ * Boundary discharge diagnostics (inflow / outflow rates are accumulated every step).
+ * volume_by_tag host [SWE_BC_MAX_TAG + 1]: volume (m^3) that has LEFT the domain through the
+ * boundary edges of each tag since swe_set_state = sum over steps and edges of dt L G~_1
+ * (negative = entered: an inflow tag with discharge Q reads -Q t; walls read 0).  Each boundary
+ * edge has one device accumulator with a single writer, summed here on the host in edge order,
+ * so the result is deterministic.  Synchronises the stream.
+ */
+int swe_get_boundary_volumes(swe_mesh *mesh, double *volume_by_tag);
+
 /* Waits for the stream. */
 int swe_sync(swe_mesh *mesh);
 
@@ -187,10 +206,12 @@ int swe_get_tile_info(const swe_mesh *mesh, int32_t *tile_cells, int64_t *ntiles
  * The tile tables themselves, for tests of the mesh builder; any pointer may be NULL.
  *   edge_a, edge_b [nedges]   end points: bits 0-28 = position in the tile's record array (local
  *                             cell index if < tile_cells, else tile_cells + index into the tile's
- *                             halo list), bits 29-30 = local edge index in that cell; edge_b = -tag
- *                             on a boundary edge; a is the end point with the smaller caller id
+ *                             halo list), bits 29-30 = local edge index in that cell; on a boundary
+ *                             edge edge_b = -(tag + 128 * boundary edge number); a is the end point
+ *                             with the smaller caller id
  *   edge_geom [nedges][3]     a's unit outward normal (n1, n2) and the edge length
- *   tinfo [ntiles][4+max_halo] {first edge, #edges, #halo ids, 0, halo ids (internal), -1 padding}
+ *   tinfo [ntiles][4+max_halo] {first edge, #edges, #halo ids, 1 if the tile has an inflow edge,
+ *                             halo ids (internal), -1 padding}
  */
 int swe_get_tile_tables(const swe_mesh *mesh, int32_t *edge_a, int32_t *edge_b, double *edge_geom,
                         int32_t *tinfo);

@@ -26,6 +26,8 @@
  *                        derivative of eq. (32) (its definition, eq. 34) on a non-uniform state
  *   whole step         : Stoker and Ritter dam-break solutions, mass conservation,
  *                        mirror symmetry
+ *   boundary volumes   : inflow tag = -Q t exactly, walls 0, tags add up to the total, volume
+ *                        change = -sum; run_until: ends on t_end, equals run() before the last step
  *   dt                 : closed form CFL * R_min / (sqrt(g h) + |V|) on a uniform state
  *   unpinned conventions: R-1 cell bed = mean of node beds, R-2 g = 9.81,
  *                        R-6 clamp in eq. (22).
@@ -64,6 +66,12 @@ typedef struct {
     int dt_valid;
     int64_t steps, nclamp;
     long double bnd_volume_out; /* cumulative sum over boundary edges of G1 * L * dt */
+    /* boundary diagnostics (inflow / outflow rates are computed every step) */
+    int64_t nb;            /* number of boundary edges */
+    int32_t *bidx;         /* [nt][3] index of the boundary edge, -1 on interior edges */
+    int32_t *btag;         /* [nb] tag of each boundary edge */
+    double *bstep;         /* [nb] G1 * L * dt of the current step */
+    long double bvol_tag[MAX_TAGS]; /* cumulative outward volume per tag */
     int nthreads;
 } oracle_mesh;
 
@@ -161,6 +169,7 @@ void oracle_destroy(oracle_mesh *m)
     free(m->tri); free(m->tag); free(m->nbr); free(m->n1); free(m->n2); free(m->len);
     free(m->area); free(m->rin); free(m->z); free(m->manning);
     free(m->h); free(m->hu); free(m->hv); free(m->h2); free(m->hu2); free(m->hv2);
+    free(m->bidx); free(m->btag); free(m->bstep);
     free(m);
 }
 
@@ -257,7 +266,16 @@ oracle_mesh *oracle_create(const double *nodes_xy, int64_t nn, const int32_t *tr
         e = f;
     }
     free(er);
-    for (int k = 0; k < MAX_TAGS; k++) m->qn_tag[k] = 0.0;
+    for (int k = 0; k < MAX_TAGS; k++) { m->qn_tag[k] = 0.0; m->bvol_tag[k] = 0.0L; }
+    /* number the boundary edges in (cell, local edge) order */
+    m->bidx = (int32_t *)malloc(sizeof(int32_t) * 3 * nt);
+    if (!m->bidx) { *err = -5; oracle_destroy(m); return NULL; }
+    m->nb = 0;
+    for (int64_t e = 0; e < 3 * nt; e++) m->bidx[e] = m->nbr[e] < 0 ? (int32_t)m->nb++ : -1;
+    m->btag = (int32_t *)malloc(sizeof(int32_t) * (m->nb > 0 ? m->nb : 1));
+    m->bstep = (double *)calloc((size_t)(m->nb > 0 ? m->nb : 1), sizeof(double));
+    if (!m->btag || !m->bstep) { *err = -5; oracle_destroy(m); return NULL; }
+    for (int64_t e = 0; e < 3 * nt; e++) if (m->bidx[e] >= 0) m->btag[m->bidx[e]] = m->tag[e];
     return m;
 }
 
@@ -286,6 +304,7 @@ void oracle_set_state(oracle_mesh *m, const double *h, const double *hu, const d
     for (int64_t i = 0; i < m->nt; i++)
         if (m->h[i] <= m->hdry) { m->hu[i] = 0.0; m->hv[i] = 0.0; }
     m->t = t0; m->dt_valid = 0; m->steps = 0; m->nclamp = 0; m->bnd_volume_out = 0.0L;
+    for (int k = 0; k < MAX_TAGS; k++) m->bvol_tag[k] = 0.0L;
 }
 
 /* CFL time step from the current state, eq.(15), R-9:
@@ -351,6 +370,7 @@ static void step(oracle_mesh *m, double dt)
                     G[1] = hL > hdry ? qn * qn / hL + 0.5 * g * hL * hL : 0.0;
                 }
                 bvol += (long double)(G[0] * m->len[3 * i + k] * dt);
+                m->bstep[m->bidx[3 * i + k]] = G[0] * m->len[3 * i + k] * dt;
             }
             /* rotate back with T^-1, eq.(12) */
             const double Fx = G[1] * n1 - G[2] * n2, Fy = G[1] * n2 + G[2] * n1;
@@ -391,6 +411,7 @@ static void step(oracle_mesh *m, double dt)
     t = m->hv; m->hv = m->hv2; m->hv2 = t;
     m->nclamp += nclamp;
     m->bnd_volume_out += bvol;
+    for (int64_t b = 0; b < m->nb; b++) m->bvol_tag[m->btag[b]] += (long double)m->bstep[b];
     m->t += dt;
     m->steps++;
 }
@@ -408,6 +429,30 @@ int64_t oracle_run(oracle_mesh *m, int64_t nsteps)
         oracle_compute_dt(m);
     }
     return done;
+}
+
+/* Steps until t >= t_end: the step that would pass t_end is shortened to end on it (the paper's
+ * runs are specified by simulated time).  At most max_steps.  Returns steps done. */
+int64_t oracle_run_until(oracle_mesh *m, double t_end, int64_t max_steps)
+{
+    int64_t done = 0;
+    if (!m->dt_valid) oracle_compute_dt(m);
+    while (done < max_steps && m->t < t_end) {
+        if (!(m->dt > 0.0)) break;
+        double dt = m->dt;
+        if (t_end - m->t < dt) dt = t_end - m->t;
+        step(m, dt);
+        oracle_compute_dt(m);
+        done++;
+    }
+    return done;
+}
+
+/* vol[MAX_TAGS]: cumulative volume (m^3) that left the domain through the boundary edges of
+ * each tag since oracle_set_state (negative = entered). */
+void oracle_get_boundary_volumes(const oracle_mesh *m, double *vol)
+{
+    for (int k = 0; k < MAX_TAGS; k++) vol[k] = (double)m->bvol_tag[k];
 }
 
 /* One step with an imposed dt (tests of the closed forms). */

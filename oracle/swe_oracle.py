@@ -33,6 +33,9 @@ def lib():
         L.oracle_run.argtypes = [C.c_void_p, i64]
         L.oracle_run.restype = i64
         L.oracle_step_dt.argtypes = [C.c_void_p, C.c_double]
+        L.oracle_run_until.argtypes = [C.c_void_p, C.c_double, i64]
+        L.oracle_run_until.restype = i64
+        L.oracle_get_boundary_volumes.argtypes = [C.c_void_p, dp]
         L.oracle_get_state.argtypes = [C.c_void_p, dp, dp, dp, dp, dp]
         L.oracle_get_stats.argtypes = [C.c_void_p, dp]
         L.oracle_get_geometry.argtypes = [C.c_void_p, C.POINTER(C.c_int64), dp, dp, dp, dp, dp, dp]
@@ -115,6 +118,15 @@ class OracleSolver:
 
     def run(self, nsteps):
         return self._L.oracle_run(self._h, int(nsteps))
+
+    def run_until(self, t_end, max_steps=1 << 40):
+        return self._L.oracle_run_until(self._h, float(t_end), int(max_steps))
+
+    def boundary_volumes(self):
+        """Cumulative outward volume (m^3) per boundary tag since set_state, array [128]."""
+        v = np.zeros(128)
+        self._L.oracle_get_boundary_volumes(self._h, _dp(v))
+        return v
 
     def step_dt(self, dt):
         self._L.oracle_step_dt(self._h, float(dt))

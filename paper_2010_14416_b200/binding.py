@@ -24,7 +24,7 @@ ERR_ALL_DRY = -9
 SYMBOLS = [
     "swe_params_default", "swe_mesh_create", "swe_mesh_destroy", "swe_mesh_workspace_bytes",
     "swe_mesh_bind_device", "swe_set_bc_value", "swe_set_state", "swe_set_state_device",
-    "swe_compute_dt", "swe_step", "swe_run", "swe_sync", "swe_get_state", "swe_get_state_device",
+    "swe_compute_dt", "swe_step", "swe_run", "swe_run_until", "swe_get_boundary_volumes", "swe_sync", "swe_get_state", "swe_get_state_device",
     "swe_get_stats", "swe_get_permutation", "swe_get_tables", "swe_get_tile_info",
     "swe_get_tile_tables", "swe_get_launch_info",
     "swe_last_error",
@@ -74,6 +74,8 @@ def load_library(rebuild_if_stale: bool = True):
     L.swe_compute_dt.argtypes = [vp, dp]
     L.swe_step.argtypes = [vp]
     L.swe_run.argtypes = [vp, i64]
+    L.swe_run_until.argtypes = [vp, C.c_double, i64, C.POINTER(C.c_int64)]
+    L.swe_get_boundary_volumes.argtypes = [vp, dp]
     L.swe_sync.argtypes = [vp]
     L.swe_get_state.argtypes = [vp, dp, dp, dp, dp, dp]
     L.swe_get_state_device.argtypes = [vp, vp, vp, vp]
@@ -201,6 +203,16 @@ class SweMesh:
 
     def run(self, nsteps):
         self._ck(self._L.swe_run(self._h, int(nsteps)))
+
+    def run_until(self, t_end, max_steps=1 << 40):
+        done = C.c_int64(0)
+        self._ck(self._L.swe_run_until(self._h, float(t_end), int(max_steps), C.byref(done)))
+        return done.value
+
+    def get_boundary_volumes(self):
+        v = np.zeros(128, dtype=np.float64)
+        self._ck(self._L.swe_get_boundary_volumes(self._h, _dp(v)))
+        return v
 
     def sync(self):
         self._ck(self._L.swe_sync(self._h))

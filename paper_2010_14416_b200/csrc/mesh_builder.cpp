@@ -232,6 +232,12 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
             return -1;
         };
         auto enc = [](int64_t p, int k) { return (int32_t)(p | ((int64_t)k << kHostIdBits)); };
+        // boundary edges numbered in (caller cell, local edge) order
+        std::vector<int32_t> bnum(3 * (size_t)nt, -1);
+        X.nbedges = 0; X.btag.clear();
+        for (size_t e = 0; e < 3 * (size_t)nt; e++)
+            if (T.nbr[e] < 0) { bnum[e] = (int32_t)X.nbedges++; X.btag.push_back(-T.nbr[e]); }
+        if (X.nbedges >= ((int64_t)1 << 24)) { err = "more than 2^24 boundary edges"; return SWE_ERR_INVALID_ARG; }
         for (int64_t t = 0; t < X.ntiles; t++) {
             const int64_t base = t * TC, nc = std::min<int64_t>(TC, nt - base);
             const size_t first = X.edges.size(), hfirst = halo.size();
@@ -254,7 +260,8 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
                     const int32_t j = T.nbr[3 * (size_t)c + k];
                     const double *nk = &T.normal[6 * (size_t)c + 2 * k];
                     if (j < 0) {                                   // boundary edge: a = this cell
-                        X.edges.push_back({ enc(q, k), j, nk[0], nk[1], T.length[3 * (size_t)c + k] });
+                        X.edges.push_back({ enc(q, k), -((-j) + 128 * bnum[3 * (size_t)c + k]), nk[0], nk[1],
+                                            T.length[3 * (size_t)c + k] });
                         continue;
                     }
                     const int64_t pj = T.inv[(size_t)j];
@@ -290,7 +297,7 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
             ti[0] = X.estart[(size_t)t]; ti[1] = X.estart[(size_t)t + 1] - X.estart[(size_t)t];
             ti[2] = nh; ti[3] = 0;
             for (int32_t e = X.estart[(size_t)t]; e < X.estart[(size_t)t + 1]; e++)
-                if (X.edges[(size_t)e].b <= -SWE_BC_INFLOW0) ti[3] = 1;      // prescribed-discharge edge
+                if (X.edges[(size_t)e].b < 0 && ((-X.edges[(size_t)e].b) & 127) >= SWE_BC_INFLOW0) ti[3] = 1;  // prescribed discharge
             std::copy(halo.begin() + hstart[(size_t)t], halo.begin() + hstart[(size_t)t + 1], ti + 4);
         }
     } catch (const std::bad_alloc &) { err = "out of host memory"; return SWE_ERR_NOMEM; }

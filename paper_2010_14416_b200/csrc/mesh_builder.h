@@ -31,7 +31,9 @@ struct HostTables {
 // once in that tile's edge list (an edge between two tiles appears in both lists).
 // Edge end points: bits 0-28 = position in the tile's record array (local cell index if
 // < tile_cells, else tile_cells + index into the tile's halo list), bits 29-30 = the edge's local
-// index k in that cell; b = -tag on a boundary edge.  a is the end point with the smaller CALLER id.
+// index k in that cell.  On a boundary edge b = -(tag + 128 * boundary edge number), the boundary
+// edges being numbered in (caller cell, local edge) order.  a is the end point with the smaller
+// CALLER id.
 struct HostEdge { int32_t a, b; double n1, n2, len; };                          // 32 bytes
 constexpr int kHostIdBits = 29;
 struct TileTables {
@@ -42,6 +44,8 @@ struct TileTables {
     // [ntiles][4 + max_halo]: {first edge, #edges, #halo ids, 1 if the tile has an inflow edge else 0,
     // halo ids (internal cell ids of the tile's off-tile end points) padded with -1}
     std::vector<int32_t> tinfo;
+    int64_t nbedges = 0;               // number of boundary edges
+    std::vector<int32_t> btag;         // [nbedges] tag of each boundary edge
     std::vector<int32_t> estart;       // [ntiles + 1] offsets into edges
     std::vector<HostEdge> edges;
     std::vector<double> cellc;         // [ntiles][3][tile_cells]: 1/|Omega|, 1/R, g m^2 (padded with 1, 1, 0)

@@ -38,7 +38,8 @@ namespace swe {
 
 struct __align__(32) Rec { double h, u, v, z; };
 
-// One edge of a tile.  a is always a cell; b is a cell or -tag on a boundary edge.  (n1,n2) is
+// One edge of a tile.  a is always a cell; b is a cell, or -(tag + 128 * boundary edge number)
+// on a boundary edge.  (n1,n2) is
 // a's unit outward normal on this edge (so b's is its negative).  a is the end point with the
 // smaller CALLER id, which makes the result independent of the renumbering (R-17).
 // Bits 0-28 of a and b: position in the tile's shared-memory record array (< tile size: the
@@ -49,9 +50,11 @@ constexpr int kIdBits = 29;
 constexpr int32_t kIdMask = (1 << kIdBits) - 1;
 
 struct Ctrl {                 // device-resident loop state
-    double t;                 // simulated time
+    double t[2];              // simulated time of the state in U0 / U1 (ping-pong like the state: every
+                              // block reads t[cur] while block 0 writes t[cur ^ 1])
     double dt;                // step the next update will use (valid after a finalise)
     double dt_last;           // step used by the latest update
+    double t_end;             // the step that would pass t_end ends on it (swe_run_until); +inf otherwise
     long long steps;
     unsigned long long n_clamped;
     int all_dry;              // set when a step found no wet cell
@@ -64,6 +67,7 @@ struct Params {
     const EdgeRec *edges;     // [estart[ntiles]] tile after tile
     const int32_t *tinfo;     // [ntiles][4 + max_halo] per-tile info block, see "the tile pipeline"
     const double *qn_tag;     // [128] unit discharge along the outward normal per inflow tag
+    double *bvol;             // [boundary edges] cumulative outward volume through each boundary edge
     double *pmax0, *pmax1;    // [npart] per-block max rate of state U0 / U1
     Ctrl *ctrl;
     int32_t nt, ntiles, npart, max_edges, max_halo;
@@ -217,7 +221,7 @@ __device__ __forceinline__ void hllc_flux(const double g, const double hg, const
 // the frame of a's outward normal n.  Side a subtracts (o0,o1,o2)/|Omega_a|, side b adds
 // (o0,o3,o4)/|Omega_b| (its outward normal is -n).
 __device__ __forceinline__ void edge_eval(const Params &P, const EdgeRec &er, const Rec &A,
-                                          const Rec &B, double o[5])
+                                          const Rec &B, const double dt, double o[5])
 {
     const double g = P.g, hg = P.hg, hdry = P.hdry;
     const double n1 = er.n1, n2 = er.n2;
@@ -235,7 +239,7 @@ __device__ __forceinline__ void edge_eval(const Params &P, const EdgeRec &er, co
         sba = hg * (hL2 - A.h * A.h);
         sbb = hg * (hR2 - B.h * B.h);
     } else {                                    // a6: boundary edge
-        const int tag = -er.b;
+        const int tag = (-er.b) & 127;
         const double hL = A.h;
         const double pr = hg * hL * hL;
         if (tag == SWE_BC_WALL) { G0 = 0.0; G1 = pr; G2 = 0.0; }                 // R-4
@@ -247,6 +251,9 @@ __device__ __forceinline__ void edge_eval(const Params &P, const EdgeRec &er, co
             G0 = qn; G2 = 0.0;
             G1 = hL > hdry ? qn * qn * fast_rcp(hL) + pr : 0.0;
         }
+        // boundary diagnostics: volume that left through this edge so far.  One
+        // writer per edge, so the sum is deterministic; walls carry no mass.
+        if (tag != SWE_BC_WALL) P.bvol[(-er.b) >> 7] += G0 * er.len * dt;
     }
     // a7: rotate back (T^-1) and scale by the edge length
     const double L = er.len;
@@ -301,6 +308,8 @@ __device__ __forceinline__ double cell_update(const Params &P, const Rec &Ui, co
     if (hn > hdry) {
         const double rhn = fast_rcp(hn);
         Un.u = qxn * rhn; Un.v = qyn * rhn;
+        // a zero step (t_end reached, swe_run_until) must not change a bit: (h u) / h is not u
+        if (dt == 0.0) { Un.u = ui; Un.v = vi; }
         // a10: local rate of the new state, eq.(15) with d = R_i
         const double ghn = g * hn, a = ghn * fast_rsqrt(ghn);
         const double v2 = Un.u * Un.u + Un.v * Un.v;
@@ -513,7 +522,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
                 int ib = TC, kb = 0;
                 if (er.b >= 0) { ib = er.b & kIdMask; kb = er.b >> kIdBits; B = srec[ib]; }
                 double o[5];
-                edge_eval(P, er, A, B, o);
+                edge_eval(P, er, A, B, dt, o);
                 if (ia < TC) {
                     double *q = so + ka * (3 * TC) + ia;
                     q[0] = o[0]; q[TC] = o[1]; q[2 * TC] = o[2];

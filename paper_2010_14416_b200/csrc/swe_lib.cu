@@ -48,7 +48,10 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
     __syncthreads();
     unsigned it = 0;
     for (long long s = 0; s < nsteps; s++) {
-        const double dt = reduce_dt(P, P.pmax(cur), s_red);
+        const double dt_cfl = reduce_dt(P, P.pmax(cur), s_red);
+        // swe_run_until: the step that would pass t_end ends on it; after that, zero steps
+        const double t_now = __ldcg(&P.ctrl->t[cur]);
+        const double dt = fmax(fmin(dt_cfl, __ldcg(&P.ctrl->t_end) - t_now), 0.0);
         unsigned nclamp = 0;
         double rate = step_tiles<TC>(P, pp, P.U(cur), P.U(cur ^ 1), dt, nclamp, it);
         rate = block_max(rate, s_red);
@@ -57,8 +60,9 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
             P.pmax(cur ^ 1)[blockIdx.x] = rate;
             if (blockIdx.x == 0) {
                 Ctrl *c = P.ctrl;
-                c->t += dt; c->dt_last = dt; c->steps += 1;
-                if (!(dt > 0.0)) c->all_dry = 1;
+                c->t[cur ^ 1] = t_now + dt;
+                if (dt > 0.0) { c->dt_last = dt; c->steps += 1; }
+                if (!(dt_cfl > 0.0)) c->all_dry = 1;
             }
         }
         cur ^= 1;
@@ -174,7 +178,7 @@ static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 namespace {
 static_assert(sizeof(HostEdge) == sizeof(EdgeRec) && kHostIdBits == kIdBits, "table records");
 struct Layout {
-    size_t U0, U1, cellc, edges, tinfo, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
+    size_t U0, U1, cellc, edges, tinfo, bvol, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
 };
 Layout make_layout(const HostTables &T, const TileTables &X)
 {
@@ -183,6 +187,7 @@ Layout make_layout(const HostTables &T, const TileTables &X)
     L.U0 = take(n * sizeof(Rec)); L.U1 = take(n * sizeof(Rec));
     L.cellc = take(X.cellc.size() * sizeof(double)); L.edges = take(X.edges.size() * sizeof(EdgeRec));
     L.tinfo = take(X.tinfo.size() * sizeof(int32_t));
+    L.bvol = take(((size_t)X.nbedges + 1) * sizeof(double));
     L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
     L.stage = take(3 * n * sizeof(double));
     L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
@@ -354,6 +359,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.U0 = (Rec *)(m->ws + L.U0); P.U1 = (Rec *)(m->ws + L.U1);
     P.cellc = (const double *)(m->ws + L.cellc); P.edges = (const EdgeRec *)(m->ws + L.edges);
     P.tinfo = (const int32_t *)(m->ws + L.tinfo);
+    P.bvol = (double *)(m->ws + L.bvol);
     m->d_zcell = (double *)(m->ws + L.zcell); m->d_inv = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
@@ -377,6 +383,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
         CK(cudaMemsetAsync(P.pmax0, 0, kMaxPart * sizeof(double), s));
         CK(cudaMemsetAsync(P.pmax1, 0, kMaxPart * sizeof(double), s));
         CK(cudaMemsetAsync(P.ctrl, 0, sizeof(Ctrl), s));
+        CK(cudaMemsetAsync(P.bvol, 0, ((size_t)X.nbedges + 1) * sizeof(double), s));
         CK(cudaStreamSynchronize(s));
     } catch (const std::bad_alloc &) { m->err = "out of host memory"; return SWE_ERR_NOMEM; }
     m->bound = true;
@@ -406,7 +413,8 @@ static int set_state_common(swe_mesh *m, const double *h, const double *hu, cons
     swe_pack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_inv, h, hu, hv, m->d_zcell);
     m->launches++;
     CK(cudaGetLastError());
-    Ctrl c{}; c.t = t0;
+    Ctrl c{}; c.t[0] = t0; c.t[1] = t0; c.t_end = INFINITY;
+    if (m->X.nbedges > 0) CK(cudaMemsetAsync(m->P.bvol, 0, (size_t)m->X.nbedges * sizeof(double), m->stream));
     CK(cudaMemcpyAsync(m->P.ctrl, &c, sizeof(Ctrl), cudaMemcpyHostToDevice, m->stream));
     CK(cudaStreamSynchronize(m->stream));
     m->have_state = true; m->have_rates = false;
@@ -546,6 +554,53 @@ int swe_run(swe_mesh *m, int64_t nsteps)
 
 int swe_step(swe_mesh *m) { return swe_run(m, 1); }
 
+int swe_run_until(swe_mesh *m, double t_end, int64_t max_steps, int64_t *steps_done)
+{
+    if (steps_done) *steps_done = 0;
+    if (!m || max_steps < 0 || !(t_end == t_end)) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
+    Ctrl c;
+    int rc = read_ctrl(m, &c, true);
+    if (rc != SWE_OK) return rc;
+    const long long steps0 = c.steps;
+    CK(cudaMemcpyAsync(&m->P.ctrl->t_end, &t_end, sizeof(double), cudaMemcpyHostToDevice, m->stream));
+    int64_t left = max_steps;
+    while (left > 0 && c.t[m->cur] < t_end && c.dt > 0.0) {
+        // the time step varies, so run the estimated number of remaining steps (zero steps after
+        // t_end is reached change nothing) and look again
+        const double est = std::ceil((t_end - c.t[m->cur]) / c.dt);
+        const int64_t chunk = std::min<int64_t>(left, est < 1.0 ? 1 : est > 128.0 ? 128 : (int64_t)est);
+        rc = swe_run(m, chunk);
+        if (rc != SWE_OK) break;
+        const long long before = c.steps;
+        rc = read_ctrl(m, &c, true);
+        if (rc != SWE_OK) break;
+        left -= c.steps - before;
+        if (c.steps == before) break;       // no progress: all dry
+    }
+    const double inf = INFINITY;
+    CK(cudaMemcpyAsync(&m->P.ctrl->t_end, &inf, sizeof(double), cudaMemcpyHostToDevice, m->stream));
+    CK(cudaStreamSynchronize(m->stream));
+    if (steps_done) *steps_done = c.steps - steps0;
+    return rc;
+}
+
+int swe_get_boundary_volumes(swe_mesh *m, double *volume_by_tag)
+{
+    if (!m || !volume_by_tag) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
+    const size_t nb = (size_t)m->X.nbedges;
+    std::vector<double> v(nb);
+    if (nb) CK(cudaMemcpyAsync(v.data(), m->P.bvol, nb * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+    CK(cudaStreamSynchronize(m->stream));
+    long double sum[SWE_BC_MAX_TAG + 1] = {};
+    for (size_t b = 0; b < nb; b++) sum[m->X.btag[b]] += (long double)v[b];
+    for (int k = 0; k <= SWE_BC_MAX_TAG; k++) volume_by_tag[k] = (double)sum[k];
+    return SWE_OK;
+}
+
 int swe_sync(swe_mesh *m)
 {
     if (!m) return SWE_ERR_INVALID_ARG;
@@ -583,7 +638,7 @@ int swe_get_state(swe_mesh *m, double *h, double *hu, double *hv, double *t, dou
     Ctrl c;
     int rc = read_ctrl(m, &c, dt_next != nullptr);
     if (rc != SWE_OK) return rc;
-    if (t) *t = c.t;
+    if (t) *t = c.t[m->cur];
     if (dt_next) *dt_next = c.dt;
     return SWE_OK;
 }
@@ -607,7 +662,7 @@ int swe_get_stats(swe_mesh *m, swe_stats *s)
         ndry += h[i] <= m->prm.h_dry;
         nbad += !(std::isfinite(h[i]) && std::isfinite(hu[i]) && std::isfinite(hv[i]));
     }
-    s->volume = (double)vol; s->t = c.t; s->dt_last = c.dt_last; s->steps = c.steps;
+    s->volume = (double)vol; s->t = c.t[m->cur]; s->dt_last = c.dt_last; s->steps = c.steps;
     s->n_dry = ndry; s->n_clamped = (int64_t)c.n_clamped; s->n_nonfinite = nbad;
     return SWE_OK;
 }

@@ -251,3 +251,38 @@ def test_random_caller_numbering_without_locality_pass():
     m2.run(200)
     for a, b in zip(m.get_state()[:3], m2.get_state()[:3]):
         np.testing.assert_array_equal(a, b)                        # R-17, bitwise
+
+
+# ---- boundary discharge diagnostics and run-until-time -------------
+@pytest.mark.parametrize("loop_mode", [B.LOOP_GRAPH, B.LOOP_PERSISTENT])
+def test_boundary_volumes_and_run_until_match_oracle(loop_mode):
+    w = W.config4(nx=320, ny=80)
+    m = B.SweMesh.from_workload(w, loop_mode=loop_mode).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    o = OracleSolver.from_workload(w)
+    t_end = 12.5
+    n_gpu, n_cpu = m.run_until(t_end), o.run_until(t_end)
+    assert n_gpu == n_cpu
+    hg, hug, hvg, tg = assert_parity(m, o, w)
+    assert tg == t_end
+    vg, vo = m.get_boundary_volumes(), o.boundary_volumes()
+    np.testing.assert_allclose(vg, vo, rtol=1e-10, atol=1e-10)
+    assert vg[W.BC_INFLOW0] == pytest.approx(-500.0 * t_end, rel=1e-12) and vg[W.BC_WALL] == 0.0
+    v0 = float(np.sum(w.h * m.get_tables()["area"]))
+    assert m.get_stats()["volume"] - v0 == pytest.approx(-vg.sum(), rel=1e-9)
+    # continuing with plain steps after run_until works (t_end is disarmed) and max_steps binds
+    assert m.run_until(1e30, max_steps=7) == 7 and o.run_until(1e30, max_steps=7) == 7
+    assert_parity(m, o, w)
+
+
+def test_config4_full_size_exact_mass_balance():
+    """13,005,000 cells, bench.py's launch configuration: after 300 steps the volume in the domain
+    has changed by exactly what crossed the boundary (inflow tag: -Q t)."""
+    w = W.config4()
+    m = B.SweMesh.from_workload(w).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    v0 = float(np.sum(w.h * m.get_tables()["area"]))
+    m.run(300)
+    st, vol = m.get_stats(), m.get_boundary_volumes()
+    assert vol[W.BC_INFLOW0] == pytest.approx(-500.0 * st["t"], rel=1e-12)
+    assert st["volume"] - v0 == pytest.approx(-vol.sum(), rel=1e-9)

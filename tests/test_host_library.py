@@ -145,6 +145,7 @@ def test_tile_tables_cover_every_cell_edge_exactly_once(ordering, block):
     nt, TC = w.ncells, X["tile_cells"]
     assert TC == block and X["ntiles"] == (nt + TC - 1) // TC
     seen = np.zeros((nt, 3), dtype=np.int32)
+    bnum = []
     mask = (1 << 29) - 1
     assert X["tinfo"][:, 0].tolist() == np.concatenate([[0], np.cumsum(X["tinfo"][:, 1])[:-1]]).tolist()
     assert X["tinfo"][:, 1].sum() == X["nedges"] and X["tinfo"][:, 1].max() == X["max_edges"]
@@ -168,8 +169,9 @@ def test_tile_tables_cover_every_cell_edge_exactly_once(ordering, block):
             if (a & mask) < TC:
                 seen[ca, ka] += 1
             if b < 0:                                                  # boundary edge
-                assert geo["nbr"][ca, ka] < 0 and -b == max(int(w.bc_tags[ca, ka]), 1)
+                assert geo["nbr"][ca, ka] < 0 and (-b) & 127 == max(int(w.bc_tags[ca, ka]), 1)
                 assert (a & mask) < TC
+                bnum.append((-b) >> 7)
                 continue
             pb, kb = internal(b & mask), b >> 29
             cb = perm[pb]
@@ -178,6 +180,7 @@ def test_tile_tables_cover_every_cell_edge_exactly_once(ordering, block):
             if (b & mask) < TC:
                 seen[cb, kb] += 1
     assert (seen == 1).all()
+    assert sorted(bnum) == list(range(int((geo["nbr"] < 0).sum())))   # boundary edges numbered once each
     # locality: a space-filling-curve order keeps most edges inside one tile
     if ordering == B.ORDER_HILBERT and block >= 192:
         assert X["edges_per_cell"] < 1.85

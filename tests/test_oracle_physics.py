@@ -258,3 +258,29 @@ def test_friction_jacobian_including_h_column_vs_symbolic_derivative():
         worst_noh = max(worst_noh, np.abs(r).max() / scale)
     assert worst < 1e-12
     assert worst_noh > 1e4 * max(worst, 1e-16)
+
+
+# ------------------------------------------------------------------ boundary diagnostics, run-until
+def test_boundary_volumes_per_tag_and_run_until():
+    """R-20 / PAPER.md:453: the inflow tag's cumulative volume is exactly -Q t, walls carry none,
+    the tags add up to the total, and the volume in the domain changes by minus that total.
+    run_until ends on t_end by shortening the last step and otherwise equals run()."""
+    w = W.config4(nx=80, ny=20)
+    s = OracleSolver.from_workload(w)
+    v0 = s.stats()["volume"]
+    n = s.run_until(30.0)
+    h, hu, hv, t, dt = s.get_state()
+    assert t == 30.0 and n == s.stats()["steps"]
+    vol = s.boundary_volumes()
+    assert vol[W.BC_INFLOW0] == pytest.approx(-500.0 * 30.0, rel=1e-12)
+    assert vol[W.BC_WALL] == 0.0 and vol[W.BC_TRANSMISSIVE] > 0.0
+    assert vol.sum() == pytest.approx(s.stats()["boundary_volume_out"], rel=1e-12)
+    assert s.stats()["volume"] - v0 == pytest.approx(-vol.sum(), rel=1e-9)
+    # the same number of plain steps reproduces every step but the shortened last one
+    r = OracleSolver.from_workload(w)
+    r.run(n - 1)
+    r2 = OracleSolver.from_workload(w)
+    r2.run_until(1e30, max_steps=n - 1)
+    for a, b in zip(r.get_state()[:4], r2.get_state()[:4]):
+        np.testing.assert_array_equal(a, b)
+    assert r.get_state()[3] < 30.0 <= r.get_state()[3] + r.get_state()[4]
