@@ -197,7 +197,7 @@ int swe_get_tables(const swe_mesh *mesh, int32_t *nbr, double *normal, double *l
  * into tiles of tile_cells consecutive cells (= swe_params.block_size); every edge touching a
  * tile is listed once in that tile (an edge between two tiles is listed in both, so
  * nedges / nt >= 1.5 measures the locality of the ordering).  max_edges / max_halo: longest edge
- * list / halo list of any tile; smem_bytes: dynamic shared memory per block.  Any pointer may be NULL.
+ * list (rounded up to an even count) / halo list of any tile; smem_bytes: dynamic shared memory per block.  Any pointer may be NULL.
  */
 int swe_get_tile_info(const swe_mesh *mesh, int32_t *tile_cells, int64_t *ntiles, int64_t *nedges,
                       int32_t *max_edges, int32_t *max_halo, size_t *smem_bytes);

@@ -220,7 +220,8 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
         X.tile_cells = TC;
         X.ntiles = (nt + TC - 1) / TC;
         X.estart.assign((size_t)X.ntiles + 1, 0);
-        std::vector<int32_t> hstart((size_t)X.ntiles + 1, 0), halo;
+        std::vector<int32_t> hstart((size_t)X.ntiles + 1, 0), halo, ecount((size_t)X.ntiles, 0);
+        X.nedges = 0;
         X.max_halo = 0;
         std::vector<int32_t> halo_tile((size_t)nt, -1), halo_slot((size_t)nt, 0);
         X.cellc.assign((size_t)X.ntiles * 3 * TC, 1.0);
@@ -260,8 +261,8 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
                     const int32_t j = T.nbr[3 * (size_t)c + k];
                     const double *nk = &T.normal[6 * (size_t)c + 2 * k];
                     if (j < 0) {                                   // boundary edge: a = this cell
-                        X.edges.push_back({ enc(q, k), -((-j) + 128 * bnum[3 * (size_t)c + k]), nk[0], nk[1],
-                                            T.length[3 * (size_t)c + k] });
+                        { const double L = T.length[3 * (size_t)c + k];
+                          X.edges.push_back({ enc(q, k), -((-j) + 128 * bnum[3 * (size_t)c + k]), L * nk[0], L * nk[1] }); }
                         continue;
                     }
                     const int64_t pj = T.inv[(size_t)j];
@@ -270,18 +271,23 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
                     const int kj = local_edge_towards(j, c);
                     if (kj < 0) { err = "inconsistent neighbour table"; return SWE_ERR_NON_MANIFOLD; }
                     if (c < j)                                     // a = smaller caller id (R-17)
-                        X.edges.push_back({ enc(q, k), enc(pos(pj), kj), nk[0], nk[1], T.length[3 * (size_t)c + k] });
+                        { const double L = T.length[3 * (size_t)c + k];
+                          X.edges.push_back({ enc(q, k), enc(pos(pj), kj), L * nk[0], L * nk[1] }); }
                     else
-                        X.edges.push_back({ enc(pos(pj), kj), enc(q, k), T.normal[6 * (size_t)j + 2 * kj],
-                                            T.normal[6 * (size_t)j + 2 * kj + 1], T.length[3 * (size_t)j + kj] });
+                        { const double L = T.length[3 * (size_t)j + kj];
+                          X.edges.push_back({ enc(pos(pj), kj), enc(q, k), L * T.normal[6 * (size_t)j + 2 * kj],
+                                              L * T.normal[6 * (size_t)j + 2 * kj + 1] }); }
                 }
                 cc[q] = 1.0 / T.area[(size_t)c];
                 cc[TC + q] = 1.0 / T.inradius[(size_t)c];
                 cc[2 * TC + q] = g * T.manning[(size_t)c] * T.manning[(size_t)c];
             }
             const size_t cnt = X.edges.size() - first;
+            ecount[(size_t)t] = (int32_t)cnt;
+            X.nedges += (int64_t)cnt;
+            if (cnt & 1) X.edges.push_back({ 0, 0, 0.0, 0.0 });       // pad to 16-byte granules
             if (X.edges.size() > (size_t)INT32_MAX) { err = "too many edges"; return SWE_ERR_INVALID_ARG; }
-            X.max_edges = std::max<int32_t>(X.max_edges, (int32_t)cnt);
+            X.max_edges = std::max<int32_t>(X.max_edges, (int32_t)(X.edges.size() - first));
             X.estart[(size_t)t + 1] = (int32_t)X.edges.size();
             if (halo.size() > (size_t)INT32_MAX) { err = "too many halo cells"; return SWE_ERR_INVALID_ARG; }
             X.max_halo = std::max<int32_t>(X.max_halo, (int32_t)(halo.size() - hfirst));
@@ -294,9 +300,9 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
         for (int64_t t = 0; t < X.ntiles; t++) {
             int32_t *ti = X.tinfo.data() + (size_t)t * stride;
             const int32_t nh = hstart[(size_t)t + 1] - hstart[(size_t)t];
-            ti[0] = X.estart[(size_t)t]; ti[1] = X.estart[(size_t)t + 1] - X.estart[(size_t)t];
+            ti[0] = X.estart[(size_t)t]; ti[1] = ecount[(size_t)t];
             ti[2] = nh; ti[3] = 0;
-            for (int32_t e = X.estart[(size_t)t]; e < X.estart[(size_t)t + 1]; e++)
+            for (int32_t e = X.estart[(size_t)t]; e < X.estart[(size_t)t] + ecount[(size_t)t]; e++)
                 if (X.edges[(size_t)e].b < 0 && ((-X.edges[(size_t)e].b) & 127) >= SWE_BC_INFLOW0) ti[3] = 1;  // prescribed discharge
             std::copy(halo.begin() + hstart[(size_t)t], halo.begin() + hstart[(size_t)t + 1], ti + 4);
         }

@@ -34,12 +34,15 @@ struct HostTables {
 // index k in that cell.  On a boundary edge b = -(tag + 128 * boundary edge number), the boundary
 // edges being numbered in (caller cell, local edge) order.  a is the end point with the smaller
 // CALLER id.
-struct HostEdge { int32_t a, b; double n1, n2, len; };                          // 32 bytes
+// (lx, ly) = edge length times a's unit outward normal.  Lists are padded to an even number of
+// records (a zero record) so that every tile's list starts and ends on a 16-byte boundary.
+struct HostEdge { int32_t a, b; double lx, ly; };                               // 24 bytes
 constexpr int kHostIdBits = 29;
 struct TileTables {
     int32_t tile_cells = 0;
     int64_t ntiles = 0;
-    int32_t max_edges = 0;             // longest edge list of any tile
+    int32_t max_edges = 0;             // longest (padded) edge list of any tile
+    int64_t nedges = 0;                // edge records without the padding
     int32_t max_halo = 0;              // longest halo list of any tile, rounded up to a multiple of 4
     // [ntiles][4 + max_halo]: {first edge, #edges, #halo ids, 1 if the tile has an inflow edge else 0,
     // halo ids (internal cell ids of the tile's off-tile end points) padded with -1}

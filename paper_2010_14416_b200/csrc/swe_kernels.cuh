@@ -38,14 +38,15 @@ namespace swe {
 
 struct __align__(32) Rec { double h, u, v, z; };
 
-// One edge of a tile.  a is always a cell; b is a cell, or -(tag + 128 * boundary edge number)
-// on a boundary edge.  (n1,n2) is
-// a's unit outward normal on this edge (so b's is its negative).  a is the end point with the
-// smaller CALLER id, which makes the result independent of the renumbering (R-17).
+// One edge of a tile (24 bytes).  a is always a cell; b is a cell, or -(tag + 128 * boundary edge
+// number) on a boundary edge.  (lx, ly) = edge length times a's unit outward normal (so b's is
+// its negative): the unit normal and the length come from one rsqrt(lx^2 + ly^2), and the
+// length-weighted flux needs neither.  a is the end point with the smaller CALLER id, which
+// makes the result independent of the renumbering (R-17).
 // Bits 0-28 of a and b: position in the tile's shared-memory record array (< tile size: the
 // tile's own cell with that local index; >= tile size: entry of the tile's halo list);
 // bits 29-30: the local edge index k of this edge in that cell.
-struct __align__(32) EdgeRec { int32_t a, b; double n1, n2, len; };
+struct __align__(8) EdgeRec { int32_t a, b; double lx, ly; };
 constexpr int kIdBits = 29;
 constexpr int32_t kIdMask = (1 << kIdBits) - 1;
 
@@ -224,7 +225,9 @@ __device__ __forceinline__ void edge_eval(const Params &P, const EdgeRec &er, co
                                           const Rec &B, const double dt, double o[5])
 {
     const double g = P.g, hg = P.hg, hdry = P.hdry;
-    const double n1 = er.n1, n2 = er.n2;
+    const double lx = er.lx, ly = er.ly;
+    const double L2 = fma(lx, lx, ly * ly), rl = fast_rsqrt(L2);
+    const double n1 = lx * rl, n2 = ly * rl;                                    // unit outward normal of a
     const double uL = fma(A.u, n1, A.v * n2), vL = fma(A.v, n1, -(A.u * n2));    // eq.(12)
     double G0, G1, G2, sba = 0.0, sbb = 0.0;
     if (er.b >= 0) {
@@ -253,15 +256,13 @@ __device__ __forceinline__ void edge_eval(const Params &P, const EdgeRec &er, co
         }
         // boundary diagnostics: volume that left through this edge so far.  One
         // writer per edge, so the sum is deterministic; walls carry no mass.
-        if (tag != SWE_BC_WALL) P.bvol[(-er.b) >> 7] += G0 * er.len * dt;
+        if (tag != SWE_BC_WALL) P.bvol[(-er.b) >> 7] += G0 * (L2 * rl) * dt;
     }
-    // a7: rotate back (T^-1) and scale by the edge length
-    const double L = er.len;
-    const double Fx = G1 * n1 - G2 * n2, Fy = G1 * n2 + G2 * n1;
-    const double Ln1 = L * n1, Ln2 = L * n2, LFx = L * Fx, LFy = L * Fy;
-    o[0] = L * G0;
-    o[1] = fma(-sba, Ln1, LFx); o[2] = fma(-sba, Ln2, LFy);
-    o[3] = fma(-sbb, Ln1, LFx); o[4] = fma(-sbb, Ln2, LFy);
+    // a7: rotate back (T^-1) and scale by the edge length: L (G1 n - G2 t) = G1 l - G2 l_perp
+    const double LFx = G1 * lx - G2 * ly, LFy = G1 * ly + G2 * lx;
+    o[0] = (L2 * rl) * G0;
+    o[1] = fma(-sba, lx, LFx); o[2] = fma(-sba, ly, LFy);
+    o[3] = fma(-sbb, lx, LFx); o[4] = fma(-sbb, ly, LFy);
 }
 
 // ---- one cell: a7-a10, eq.(37), PAPER.md:250 ---------------------------------------------------
@@ -365,34 +366,39 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 // Shared memory of one block (dynamic); TC = blockDim.x, ME = P.max_edges:
 //   double  so[9][TC]              (local edge k, component) flux slots of the tile's cells
 //   Rec     srec[2][TC + MH]       state records of the tile's cells, then of its halo cells
-//   EdgeRec sedge[ME]              the tile's edge list
+//   EdgeRec sedge[2][ME]           the tile's edge list (24-byte records, ME even)
 //   double  scell[3][TC]           1/|Omega|, 1/R, g m^2
 //   int32   sinfo[3][4 + MH]       info blocks (three tiles deep)
-//   uint64  bar[6]                 rec[2], info[3], edge[1]
-// Schedule for the block's n-th tile (s = n & 1), all copies asynchronous:
-//   top      wait: own halo gathers of tile n, records of tile n, edge list of tile n; barrier
-//            issue: records of tile n+1 (bulk) -> srec[s^1]; info block of tile n+2 (bulk);
-//                   cell constants of tile n (cp.async); halo gathers of tile n+1 (cp.async,
-//                   its info block landed one tile ago) -> srec[s^1][TC..]
+//   uint64  bar[7]                 rec[2], info[3], edge[2]
+// Schedule for the block's n-th tile (s = n & 1), all copies asynchronous and one tile ahead
+// (measured: with the edge list issued only after the edge phase, blocks spent 26 % of their
+// time waiting for it):
+//   top      wait: own halo gathers, records and edge list of tile n; barrier (= the dry vote)
+//            issue: records of tile n+1 (bulk) -> srec[s^1]; edge list of tile n+1 (bulk) ->
+//                   sedge[s^1]; info block of tile n+2 (bulk); cell constants of tile n
+//                   (cp.async); halo gathers of tile n+1 (cp.async, its info block landed one
+//                   tile ago) -> srec[s^1][TC..]
 //   phase 1  edges: shared memory only
-//   mid      barrier; issue: edge list of tile n+1 (bulk) into the single edge buffer
+//   mid      barrier
 //   phase 2  cells
 constexpr int kInfoHdr = 4;
-constexpr int kNumBars = 6;
+constexpr int kNumBars = 7;
 __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int ME)
 {
     return (size_t)TC * 9 * sizeof(double) + 2 * (size_t)(TC + MH) * sizeof(Rec) +
-           (size_t)ME * sizeof(EdgeRec) + (size_t)TC * 3 * sizeof(double) +
+           2 * (size_t)ME * sizeof(EdgeRec) + (size_t)TC * 3 * sizeof(double) +
            3 * (size_t)(kInfoHdr + MH) * sizeof(int32_t) + kNumBars * sizeof(uint64_t);
 }
 template <int TC> struct TilePipe {
-    double *so; Rec *srec0; EdgeRec *sedge; double *scell; int32_t *sinfo0; uint64_t *bar;
+    double *so; Rec *srec0; EdgeRec *sedge0; double *scell; int32_t *sinfo0; uint64_t *bar;
+    int edge_stride;
+    __device__ __forceinline__ EdgeRec *sedge(int s) const { return sedge0 + s * edge_stride; }
     int rec_stride, info_stride;
     __device__ __forceinline__ Rec *srec(int s) const { return srec0 + s * rec_stride; }
     __device__ __forceinline__ int32_t *sinfo(int j) const { return sinfo0 + j * info_stride; }
     __device__ __forceinline__ uint64_t *rbar(int s) const { return bar + s; }
     __device__ __forceinline__ uint64_t *ibar(int j) const { return bar + 2 + j; }
-    __device__ __forceinline__ uint64_t *ebar() const { return bar + 5; }
+    __device__ __forceinline__ uint64_t *ebar(int s) const { return bar + 5 + s; }
 };
 template <int TC> __device__ __forceinline__ TilePipe<TC> make_pipe(const Params &P, unsigned char *smem)
 {
@@ -400,7 +406,8 @@ template <int TC> __device__ __forceinline__ TilePipe<TC> make_pipe(const Params
     p.rec_stride = TC + P.max_halo; p.info_stride = kInfoHdr + P.max_halo;
     p.so = reinterpret_cast<double *>(smem);                 smem += (size_t)TC * 9 * sizeof(double);
     p.srec0 = reinterpret_cast<Rec *>(smem);                 smem += 2 * (size_t)p.rec_stride * sizeof(Rec);
-    p.sedge = reinterpret_cast<EdgeRec *>(smem);             smem += (size_t)P.max_edges * sizeof(EdgeRec);
+    p.sedge0 = reinterpret_cast<EdgeRec *>(smem);            smem += 2 * (size_t)P.max_edges * sizeof(EdgeRec);
+    p.edge_stride = P.max_edges;
     p.scell = reinterpret_cast<double *>(smem);              smem += (size_t)TC * 3 * sizeof(double);
     p.sinfo0 = reinterpret_cast<int32_t *>(smem);            smem += 3 * (size_t)p.info_stride * sizeof(int32_t);
     p.bar = reinterpret_cast<uint64_t *>(smem);
@@ -416,10 +423,11 @@ template <int TC> __device__ __forceinline__ void issue_recs(const Params &P, co
     bulk_g2s(pp.srec(s), Uin + base, (unsigned)nc * sizeof(Rec), pp.rbar(s));
 }
 template <int TC> __device__ __forceinline__ void issue_edges(const Params &P, const TilePipe<TC> &pp,
-                                                              const int e0, const int ne)
+                                                              const int e0, const int ne, const int s)
 {
-    mbar_expect_tx(pp.ebar(), (unsigned)ne * sizeof(EdgeRec));
-    bulk_g2s(pp.sedge, P.edges + e0, (unsigned)ne * sizeof(EdgeRec), pp.ebar());
+    const unsigned bytes = (unsigned)((ne + 1) & ~1) * sizeof(EdgeRec);      // lists are padded to 16 bytes
+    mbar_expect_tx(pp.ebar(s), bytes);
+    bulk_g2s(pp.sedge(s), P.edges + e0, bytes, pp.ebar(s));
 }
 template <int TC> __device__ __forceinline__ void issue_info(const Params &P, const TilePipe<TC> &pp,
                                                              const int tile, const int j)
@@ -460,14 +468,13 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
         issue_info(P, pp, tile, n % 3);
         issue_recs(P, pp, Uin, tile, n & 1);
         const int32_t *gi = P.tinfo + (size_t)tile * pp.info_stride;
-        issue_edges(P, pp, __ldg(gi), __ldg(gi + 1));
+        issue_edges(P, pp, __ldg(gi), __ldg(gi + 1), n & 1);
         if (tile + G < P.ntiles) issue_info(P, pp, tile + G, (n + 1) % 3);
     }
     mbar_wait(pp.ibar(n % 3), (n / 3) & 1u);
     gather_halo(pp, Uin, n % 3, n & 1);
     cp_async_commit();
     double *const so = pp.so;
-    const EdgeRec *const sedge = pp.sedge;
     for (; tile < P.ntiles; tile += G, n++) {
         const int s = n & 1;
         const int base = tile * TC;
@@ -475,8 +482,9 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
         // ---- top
         cp_async_wait<0>();                               // own halo gathers of this tile
         mbar_wait(pp.rbar(s), (n >> 1) & 1u);
-        mbar_wait(pp.ebar(), n & 1u);
+        mbar_wait(pp.ebar(s), (n >> 1) & 1u);
         const Rec *const srec = pp.srec(s);
+        const EdgeRec *const sedge = pp.sedge(s);
         const int32_t *const info = pp.sinfo(n % 3);
         const int ne = info[1], nh = info[2];
         // is anything wet in the tile or its halo?  Each thread looks at its own record and at
@@ -500,6 +508,10 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
         cp_async_commit();
         if (have_next) {
             mbar_wait(pp.ibar((n + 1) % 3), ((n + 1) / 3) & 1u);
+            if (tid == 0) {
+                const int32_t *ni = pp.sinfo((n + 1) % 3);
+                issue_edges(P, pp, ni[0], ni[1], s ^ 1);
+            }
             gather_halo(pp, Uin, (n + 1) % 3, s ^ 1);
         }
         cp_async_commit();
@@ -507,10 +519,6 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
             // Every cell of the tile and every neighbour is dry and no discharge is prescribed:
             // all fluxes vanish, h' = h + 0, and dry cells carry u = v = 0 already (R-15), so the
             // step leaves the records unchanged bit for bit.  The copy still moves them.
-            if (tid == 0 && have_next) {
-                const int32_t *ni = pp.sinfo((n + 1) % 3);
-                issue_edges(P, pp, ni[0], ni[1]);
-            }
             if (i < P.nt) store_rec(Uout + i, srec[tid]);
         } else {
             // ---- phase 1: every edge of the tile once, shared memory only
@@ -534,10 +542,6 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
             }
             cp_async_wait<1>();                               // this tile's cell constants
             __syncthreads();
-            if (tid == 0 && have_next) {
-                const int32_t *ni = pp.sinfo((n + 1) % 3);
-                issue_edges(P, pp, ni[0], ni[1]);
-            }
             // ---- phase 2: every cell of the tile
             if (i < P.nt) {
                 const Rec Ui = srec[tid];

@@ -285,7 +285,7 @@ int swe_get_tile_info(const swe_mesh *m, int32_t *tile_cells, int64_t *ntiles, i
     if (!m) return SWE_ERR_INVALID_ARG;
     if (tile_cells) *tile_cells = m->X.tile_cells;
     if (ntiles) *ntiles = m->X.ntiles;
-    if (nedges) *nedges = (int64_t)m->X.edges.size();
+    if (nedges) *nedges = m->X.nedges;
     if (max_edges) *max_edges = m->X.max_edges;
     if (max_halo) *max_halo = m->X.max_halo;
     if (smem_bytes) *smem_bytes = tile_smem_bytes(m->X.tile_cells, m->X.max_halo, m->X.max_edges);
@@ -295,14 +295,26 @@ int swe_get_tile_info(const swe_mesh *m, int32_t *tile_cells, int64_t *ntiles, i
 int swe_get_tile_tables(const swe_mesh *m, int32_t *edge_a, int32_t *edge_b, double *edge_geom, int32_t *tinfo)
 {
     if (!m) return SWE_ERR_INVALID_ARG;
-    const size_t ne = m->X.edges.size();
-    for (size_t e = 0; e < ne; e++) {
-        const HostEdge &E = m->X.edges[e];
-        if (edge_a) edge_a[e] = E.a;
-        if (edge_b) edge_b[e] = E.b;
-        if (edge_geom) { edge_geom[3 * e] = E.n1; edge_geom[3 * e + 1] = E.n2; edge_geom[3 * e + 2] = E.len; }
+    // records without the padding, tile after tile; tinfo[.][0] is rewritten to index this list
+    const size_t stride = 4 + (size_t)m->X.max_halo;
+    size_t o = 0;
+    for (int64_t t = 0; t < m->X.ntiles; t++) {
+        const int32_t *ti = m->X.tinfo.data() + (size_t)t * stride;
+        for (int32_t k = 0; k < ti[1]; k++, o++) {
+            const HostEdge &E = m->X.edges[(size_t)ti[0] + k];
+            if (edge_a) edge_a[o] = E.a;
+            if (edge_b) edge_b[o] = E.b;
+            if (edge_geom) {
+                const double L = std::sqrt(E.lx * E.lx + E.ly * E.ly);
+                edge_geom[3 * o] = E.lx / L; edge_geom[3 * o + 1] = E.ly / L; edge_geom[3 * o + 2] = L;
+            }
+        }
     }
-    if (tinfo) std::memcpy(tinfo, m->X.tinfo.data(), m->X.tinfo.size() * sizeof(int32_t));
+    if (tinfo) {
+        std::memcpy(tinfo, m->X.tinfo.data(), m->X.tinfo.size() * sizeof(int32_t));
+        int32_t first = 0;
+        for (int64_t t = 0; t < m->X.ntiles; t++) { tinfo[(size_t)t * stride] = first; first += tinfo[(size_t)t * stride + 1]; }
+    }
     return SWE_OK;
 }
 

@@ -148,7 +148,7 @@ def test_tile_tables_cover_every_cell_edge_exactly_once(ordering, block):
     bnum = []
     mask = (1 << 29) - 1
     assert X["tinfo"][:, 0].tolist() == np.concatenate([[0], np.cumsum(X["tinfo"][:, 1])[:-1]]).tolist()
-    assert X["tinfo"][:, 1].sum() == X["nedges"] and X["tinfo"][:, 1].max() == X["max_edges"]
+    assert X["tinfo"][:, 1].sum() == X["nedges"] and (X["tinfo"][:, 1].max() + 1) // 2 * 2 == X["max_edges"]   # lists are padded to even length
     for t in range(X["ntiles"]):
         e0, ne, nh = X["tinfo"][t, :3]
         halo = X["tinfo"][t, 4:4 + nh]
