@@ -364,7 +364,9 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 //   [0] first edge of the tile in P.edges   [1] number of edges   [2] number of halo ids
 //   [3] 1 if an inflow edge touches it      [4..] halo ids (internal cell ids), padded with -1
 // Shared memory of one block (dynamic); TC = blockDim.x, ME = P.max_edges:
-//   double  so[9][TC]              (local edge k, component) flux slots of the tile's cells
+//   double  so[3][3 TC + 5]        (local edge k)(component, cell) flux slots of the tile's cells; the 5
+//                                  doubles of padding put the three slots of one cell in different banks
+//                                  (two edges of a cell are usually evaluated by adjacent lanes)
 //   Rec     srec[2][TC + MH]       state records of the tile's cells, then of its halo cells
 //   EdgeRec sedge[2][ME]           the tile's edge list (24-byte records, ME even)
 //   double  scell[3][TC]           1/|Omega|, 1/R, g m^2
@@ -382,10 +384,11 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 //   mid      barrier
 //   phase 2  cells
 constexpr int kInfoHdr = 4;
+template <int TC> struct SlotLayout { static constexpr int plane = 3 * TC + 5; static constexpr int doubles = 3 * plane + 4; };
 constexpr int kNumBars = 7;
 __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int ME)
 {
-    return (size_t)TC * 9 * sizeof(double) + 2 * (size_t)(TC + MH) * sizeof(Rec) +
+    return ((size_t)TC * 9 + 28) * sizeof(double) + 2 * (size_t)(TC + MH) * sizeof(Rec) +
            2 * (size_t)ME * sizeof(EdgeRec) + (size_t)TC * 3 * sizeof(double) +
            3 * (size_t)(kInfoHdr + MH) * sizeof(int32_t) + kNumBars * sizeof(uint64_t);
 }
@@ -404,7 +407,7 @@ template <int TC> __device__ __forceinline__ TilePipe<TC> make_pipe(const Params
 {
     TilePipe<TC> p;
     p.rec_stride = TC + P.max_halo; p.info_stride = kInfoHdr + P.max_halo;
-    p.so = reinterpret_cast<double *>(smem);                 smem += (size_t)TC * 9 * sizeof(double);
+    p.so = reinterpret_cast<double *>(smem);                 smem += ((size_t)TC * 9 + 28) * sizeof(double);
     p.srec0 = reinterpret_cast<Rec *>(smem);                 smem += 2 * (size_t)p.rec_stride * sizeof(Rec);
     p.sedge0 = reinterpret_cast<EdgeRec *>(smem);            smem += 2 * (size_t)P.max_edges * sizeof(EdgeRec);
     p.edge_stride = P.max_edges;
@@ -443,7 +446,7 @@ template <int TC> __device__ __forceinline__ void gather_halo(const TilePipe<TC>
     const int32_t *info = pp.sinfo(j);
     const int nh = info[2];
     Rec *dst = pp.srec(s) + TC;
-    for (int q = threadIdx.x; q < nh; q += TC) {
+    for (int q = TC - 1 - (int)threadIdx.x; q < nh; q += TC) {        // last warps first: they have slack
         const char *src = reinterpret_cast<const char *>(Uin + info[kInfoHdr + q]);
         cp_async16(reinterpret_cast<char *>(dst + q), src);
         cp_async16(reinterpret_cast<char *>(dst + q) + 16, src + 16);
@@ -464,7 +467,11 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
     int tile = blockIdx.x;
     if (tile >= P.ntiles) return 0.0;
     // ---- prologue: everything tile n needs, and the info block of tile n+1
-    if (tid == 0) {
+    // the copies are issued by lane 0 of the LAST warp: the edge loop gives the first warps one more
+    // iteration than the last ones (ne ~ 1.66 TC), so the last warp has the slack (measured: with
+    // thread 0 as producer warp 0 reached the mid barrier ~1000 cycles late)
+    const bool producer = tid == TC - 32;
+    if (producer) {
         issue_info(P, pp, tile, n % 3);
         issue_recs(P, pp, Uin, tile, n & 1);
         const int32_t *gi = P.tinfo + (size_t)tile * pp.info_stride;
@@ -492,11 +499,11 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
         const int i = base + tid;
         bool wet = i < P.nt && srec[tid].h > P.hdry;
         if (!wet)       // a wet own cell already decides the vote
-            for (int q = tid; q < nh; q += TC) wet |= srec[TC + q].h > P.hdry;
+            for (int q = TC - 1 - tid; q < nh; q += TC) wet |= srec[TC + q].h > P.hdry;
         // barrier: everyone has left the previous tile; everyone's gathers are visible
         // (the warp vote only tells the compiler that the outcome is warp-uniform)
         const bool active = __any_sync(0xffffffffu, __syncthreads_or(wet) || info[3] != 0);
-        if (tid == 0 && have_next) {
+        if (producer && have_next) {
             issue_recs(P, pp, Uin, tile + G, s ^ 1);
             if (tile + 2 * G < P.ntiles) issue_info(P, pp, tile + 2 * G, (n + 2) % 3);
         }
@@ -508,7 +515,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
         cp_async_commit();
         if (have_next) {
             mbar_wait(pp.ibar((n + 1) % 3), ((n + 1) / 3) & 1u);
-            if (tid == 0) {
+            if (producer) {
                 const int32_t *ni = pp.sinfo((n + 1) % 3);
                 issue_edges(P, pp, ni[0], ni[1], s ^ 1);
             }
@@ -532,11 +539,11 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
                 double o[5];
                 edge_eval(P, er, A, B, dt, o);
                 if (ia < TC) {
-                    double *q = so + ka * (3 * TC) + ia;
+                    double *q = so + ka * SlotLayout<TC>::plane + ia;
                     q[0] = o[0]; q[TC] = o[1]; q[2 * TC] = o[2];
                 }
                 if (ib < TC) {
-                    double *q = so + kb * (3 * TC) + ib;
+                    double *q = so + kb * SlotLayout<TC>::plane + ib;
                     q[0] = -o[0]; q[TC] = -o[3]; q[2 * TC] = -o[4];
                 }
             }
@@ -548,9 +555,10 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
                 const double *sc = pp.scell + tid;
                 const double *q = so + tid;
                 // three edges in the fixed order k = 0,1,2 (R-17)
-                const double s1 = (q[0] + q[3 * TC]) + q[6 * TC];
-                const double s2 = (q[TC] + q[4 * TC]) + q[7 * TC];
-                const double s3 = (q[2 * TC] + q[5 * TC]) + q[8 * TC];
+                constexpr int PL = SlotLayout<TC>::plane;
+                const double s1 = (q[0] + q[PL]) + q[2 * PL];
+                const double s2 = (q[TC] + q[PL + TC]) + q[2 * PL + TC];
+                const double s3 = (q[2 * TC] + q[PL + 2 * TC]) + q[2 * PL + 2 * TC];
                 Rec Un;
                 rate = fmax(rate, cell_update(P, Ui, s1, s2, s3, sc[0], sc[TC], sc[2 * TC], dt, Un, nclamp));
                 store_rec(Uout + i, Un);
