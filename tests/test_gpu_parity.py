@@ -286,3 +286,40 @@ def test_config4_full_size_exact_mass_balance():
     st, vol = m.get_stats(), m.get_boundary_volumes()
     assert vol[W.BC_INFLOW0] == pytest.approx(-500.0 * st["t"], rel=1e-12)
     assert st["volume"] - v0 == pytest.approx(-vol.sum(), rel=1e-9)
+
+
+@pytest.mark.parametrize("block_size", [64, 128, 256])
+def test_other_tile_sizes(block_size):
+    """Every supported tile size (threads per block) gives the default's bits: the tile decomposition
+    only changes who evaluates an edge, never how (R-17, R-23)."""
+    w = W.config4(nx=200, ny=50)
+    ref = B.SweMesh.from_workload(w).bind_device()
+    ref.set_state(w.h, w.hu, w.hv)
+    ref.run(150)
+    m = B.SweMesh.from_workload(w, block_size=block_size).bind_device()
+    assert m.get_launch_info()["block"] == block_size
+    m.set_state(w.h, w.hu, w.hv)
+    m.run(150)
+    for a, b in zip(ref.get_state()[:3], m.get_state()[:3]):
+        np.testing.assert_array_equal(a, b)
+
+
+def test_zero_threshold_and_zero_steps():
+    """h_dry = 0 (the library floors it at 1e-250 so that every rsqrt argument stays normal) and
+    swe_run(0) / a reached t_end leave the state bitwise unchanged."""
+    w = W.canal_dam_break(60, 6, h_right=0.0, manning=0.03, length=60.0, seed=21)
+    w.h_dry = 0.0
+    m, o = run_both(w, 120)
+    hg, hug, hvg, tg, _ = m.get_state()
+    ho, huo, hvo, to, _ = o.get_state()
+    np.testing.assert_allclose(hg, ho, rtol=RTOL, atol=ATOL)
+    np.testing.assert_allclose(hug, huo, rtol=RTOL, atol=ATOL)
+    np.testing.assert_allclose(hvg, hvo, rtol=RTOL, atol=ATOL)
+    assert tg == pytest.approx(to, rel=1e-12) and np.isfinite(hg).all()
+    before = m.get_state()
+    m.run(0)
+    assert m.run_until(before[3]) == 0          # t_end already reached: no step
+    after = m.get_state()
+    for a, b in zip(before[:3], after[:3]):
+        np.testing.assert_array_equal(a, b)
+    assert before[3] == after[3]
