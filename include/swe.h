@@ -124,8 +124,9 @@ int swe_set_bc_value(swe_mesh *mesh, int tag, double total_discharge);
 
 /*
  * Sets U = (h, hu, hv) and the time.  host / device [nt] each, caller numbering.  Requires
- * h >= 0 and finite values (checked on the host variant).  Momentum of dry cells (h <= h_dry)
- * is discarded (R-15).  Resets the step counter; the time step becomes stale.
+ * h >= 0 and finite values (both variants check this on the device while converting; on
+ * SWE_ERR_BAD_VALUE the handle is left without a state).  Momentum of dry cells (h <= h_dry)
+ * is discarded (R-15).  Resets the step counter and the boundary volumes; the time step becomes stale.
  */
 int swe_set_state(swe_mesh *mesh, const double *h, const double *hu, const double *hv, double t0);
 int swe_set_state_device(swe_mesh *mesh, const double *d_h, const double *d_hu, const double *d_hv,

@@ -59,7 +59,7 @@ struct Ctrl {                 // device-resident loop state
     long long steps;
     unsigned long long n_clamped;
     int all_dry;              // set when a step found no wet cell
-    int pad;
+    int bad_cell;             // smallest caller id with a negative depth or a non-finite value (swe_set_state)
 };
 
 struct Params {

@@ -123,7 +123,11 @@ __global__ void swe_pack_kernel(const Params P, const int cur, const int32_t *__
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.nt) return;
     Rec r; r.h = h[c]; r.z = zcell[c];
-    if (r.h > P.hdry) { r.u = hu[c] / r.h; r.v = hv[c] / r.h; } else { r.u = 0.0; r.v = 0.0; }
+    const double qx = hu[c], qy = hv[c];
+    // validation on the device: the state is here anyway, and a host loop over three arrays
+    // would cost more than the copy
+    if (!(r.h >= 0.0) || !isfinite(r.h) || !isfinite(qx) || !isfinite(qy)) atomicMin(&P.ctrl->bad_cell, c);
+    if (r.h > P.hdry) { r.u = qx / r.h; r.v = qy / r.h; } else { r.u = 0.0; r.v = 0.0; }
     store_rec(P.U(cur) + inv[c], r);
 }
 __global__ void swe_unpack_kernel(const Params P, const int cur, const int32_t *__restrict__ inv,
@@ -422,14 +426,20 @@ static int set_state_common(swe_mesh *m, const double *h, const double *hu, cons
 {
     const int n = (int)m->T.nt;
     m->cur = 0;
+    m->have_state = false; m->have_rates = false;
+    Ctrl c{}; c.t[0] = t0; c.t[1] = t0; c.t_end = INFINITY; c.bad_cell = INT32_MAX;
+    if (m->X.nbedges > 0) CK(cudaMemsetAsync(m->P.bvol, 0, (size_t)m->X.nbedges * sizeof(double), m->stream));
+    CK(cudaMemcpyAsync(m->P.ctrl, &c, sizeof(Ctrl), cudaMemcpyHostToDevice, m->stream));
     swe_pack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_inv, h, hu, hv, m->d_zcell);
     m->launches++;
     CK(cudaGetLastError());
-    Ctrl c{}; c.t[0] = t0; c.t[1] = t0; c.t_end = INFINITY;
-    if (m->X.nbedges > 0) CK(cudaMemsetAsync(m->P.bvol, 0, (size_t)m->X.nbedges * sizeof(double), m->stream));
-    CK(cudaMemcpyAsync(m->P.ctrl, &c, sizeof(Ctrl), cudaMemcpyHostToDevice, m->stream));
+    CK(cudaMemcpyAsync(&c, m->P.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, m->stream));
     CK(cudaStreamSynchronize(m->stream));
-    m->have_state = true; m->have_rates = false;
+    if (c.bad_cell != INT32_MAX) {
+        m->err = "state has a negative depth or a non-finite value at cell " + std::to_string(c.bad_cell);
+        return SWE_ERR_BAD_VALUE;
+    }
+    m->have_state = true;
     return SWE_OK;
 }
 
@@ -438,12 +448,6 @@ int swe_set_state(swe_mesh *m, const double *h, const double *hu, const double *
     if (!m || !h || !hu || !hv || !std::isfinite(t0)) return SWE_ERR_INVALID_ARG;
     if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
     const size_t n = (size_t)m->T.nt;
-    for (size_t i = 0; i < n; i++) {
-        if (!(h[i] >= 0.0) || !std::isfinite(h[i]) || !std::isfinite(hu[i]) || !std::isfinite(hv[i])) {
-            m->err = "state has a negative depth or a non-finite value at cell " + std::to_string(i);
-            return SWE_ERR_BAD_VALUE;
-        }
-    }
     double *st = m->d_stage;
     CK(cudaMemcpyAsync(st, h, n * sizeof(double), cudaMemcpyHostToDevice, m->stream));
     CK(cudaMemcpyAsync(st + n, hu, n * sizeof(double), cudaMemcpyHostToDevice, m->stream));
