@@ -179,6 +179,17 @@ int swe_sync(swe_mesh *mesh);
 int swe_get_state(swe_mesh *mesh, double *h, double *hu, double *hv, double *t, double *dt_next);
 int swe_get_state_device(swe_mesh *mesh, double *d_h, double *d_hu, double *d_hv);
 
+/*
+ * Asynchronous snapshot (PAPER.md:453 uses a side stream for its per-step diagnostics): the
+ * current state is converted on the mesh's stream and then copied to the host buffers on a side
+ * stream, while steps queued after this call run concurrently.  h, hu, hv host [nt] (pinned
+ * memory for a truly asynchronous copy), t host (may be NULL): valid after swe_snapshot_wait (or
+ * the next swe_snapshot_begin / swe_get_state / swe_set_state / swe_mesh_destroy on this handle,
+ * which wait for it).  One snapshot can be pending per handle.
+ */
+int swe_snapshot_begin(swe_mesh *mesh, double *h, double *hu, double *hv, double *t);
+int swe_snapshot_wait(swe_mesh *mesh);
+
 /* Diagnostics (synchronises, copies h to the host). */
 int swe_get_stats(swe_mesh *mesh, swe_stats *stats);
 

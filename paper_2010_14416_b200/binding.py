@@ -24,7 +24,8 @@ ERR_ALL_DRY = -9
 SYMBOLS = [
     "swe_params_default", "swe_mesh_create", "swe_mesh_destroy", "swe_mesh_workspace_bytes",
     "swe_mesh_bind_device", "swe_set_bc_value", "swe_set_state", "swe_set_state_device",
-    "swe_compute_dt", "swe_step", "swe_run", "swe_run_until", "swe_get_boundary_volumes", "swe_sync", "swe_get_state", "swe_get_state_device",
+    "swe_compute_dt", "swe_step", "swe_run", "swe_run_until", "swe_get_boundary_volumes",
+    "swe_snapshot_begin", "swe_snapshot_wait", "swe_sync", "swe_get_state", "swe_get_state_device",
     "swe_get_stats", "swe_get_permutation", "swe_get_tables", "swe_get_tile_info",
     "swe_get_tile_tables", "swe_get_launch_info",
     "swe_last_error",
@@ -76,6 +77,8 @@ def load_library(rebuild_if_stale: bool = True):
     L.swe_run.argtypes = [vp, i64]
     L.swe_run_until.argtypes = [vp, C.c_double, i64, C.POINTER(C.c_int64)]
     L.swe_get_boundary_volumes.argtypes = [vp, dp]
+    L.swe_snapshot_begin.argtypes = [vp, dp, dp, dp, dp]
+    L.swe_snapshot_wait.argtypes = [vp]
     L.swe_sync.argtypes = [vp]
     L.swe_get_state.argtypes = [vp, dp, dp, dp, dp, dp]
     L.swe_get_state_device.argtypes = [vp, vp, vp, vp]
@@ -104,9 +107,9 @@ class SweMesh:
 
     def __init__(self, nodes_xy, tris, bathymetry, manning, bc_tags, *, g=9.81, cfl=0.9,
                  h_dry=1e-6, ordering=ORDER_HILBERT, block_size=0, loop_mode=LOOP_AUTO):
+        self._h = None
         L = load_library()
         self._L = L
-        self._h = None
         xy = np.ascontiguousarray(nodes_xy, dtype=np.float64)
         tr = np.ascontiguousarray(tris, dtype=np.int32)
         zz = np.ascontiguousarray(bathymetry, dtype=np.float64)
@@ -213,6 +216,16 @@ class SweMesh:
         v = np.zeros(128, dtype=np.float64)
         self._ck(self._L.swe_get_boundary_volumes(self._h, _dp(v)))
         return v
+
+    def snapshot_begin(self, h, hu, hv):
+        """Asynchronous snapshot into the given float64 arrays (pinned for a real overlap)."""
+        self._snap_t = C.c_double(0.0)
+        self._snap_bufs = (h, hu, hv)      # keep them alive until snapshot_wait
+        self._ck(self._L.swe_snapshot_begin(self._h, _dp(h), _dp(hu), _dp(hv), C.byref(self._snap_t)))
+
+    def snapshot_wait(self):
+        self._ck(self._L.swe_snapshot_wait(self._h))
+        return self._snap_t.value
 
     def sync(self):
         self._ck(self._L.swe_sync(self._h))

@@ -164,6 +164,9 @@ struct swe_mesh {
     int64_t launches = 0;
     double qn_tag[SWE_BC_MAX_TAG + 1] = {};
     std::map<std::pair<int, int>, cudaGraphExec_t> graphs; // (steps, cur) -> exec
+    // asynchronous snapshot (side stream)
+    cudaStream_t side = nullptr; cudaEvent_t ev_ready = nullptr, ev_done = nullptr;
+    bool snap_pending = false; double *snap_t = nullptr; Ctrl *snap_ctrl = nullptr /* pinned */; int snap_cur = 0;
 };
 
 static thread_local std::string g_create_err;
@@ -251,6 +254,11 @@ int swe_mesh_destroy(swe_mesh *m)
 {
     if (!m) return SWE_OK;
     for (auto &kv : m->graphs) cudaGraphExecDestroy(kv.second);
+    if (m->snap_pending) cudaEventSynchronize(m->ev_done);
+    if (m->ev_ready) cudaEventDestroy(m->ev_ready);
+    if (m->ev_done) cudaEventDestroy(m->ev_done);
+    if (m->side) cudaStreamDestroy(m->side);
+    if (m->snap_ctrl) cudaFreeHost(m->snap_ctrl);
     delete m;
     return SWE_OK;
 }
@@ -422,6 +430,8 @@ int swe_set_bc_value(swe_mesh *m, int tag, double total_discharge)
     return SWE_OK;
 }
 
+static int snapshot_finish(swe_mesh *m);
+
 static int set_state_common(swe_mesh *m, const double *h, const double *hu, const double *hv, double t0)
 {
     const int n = (int)m->T.nt;
@@ -449,6 +459,7 @@ int swe_set_state(swe_mesh *m, const double *h, const double *hu, const double *
     if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
     const size_t n = (size_t)m->T.nt;
     double *st = m->d_stage;
+    { int rc = snapshot_finish(m); if (rc != SWE_OK) return rc; }
     CK(cudaMemcpyAsync(st, h, n * sizeof(double), cudaMemcpyHostToDevice, m->stream));
     CK(cudaMemcpyAsync(st + n, hu, n * sizeof(double), cudaMemcpyHostToDevice, m->stream));
     CK(cudaMemcpyAsync(st + 2 * n, hv, n * sizeof(double), cudaMemcpyHostToDevice, m->stream));
@@ -637,6 +648,53 @@ int swe_get_state_device(swe_mesh *m, double *d_h, double *d_hu, double *d_hv)
     return SWE_OK;
 }
 
+// the staging buffer is shared by swe_set_state, swe_get_state and the snapshot: finish a
+// pending snapshot before anyone else writes it
+static int snapshot_finish(swe_mesh *m)
+{
+    if (!m->snap_pending) return SWE_OK;
+    CK(cudaEventSynchronize(m->ev_done));
+    m->snap_pending = false;
+    if (m->snap_t) *m->snap_t = m->snap_ctrl->t[m->snap_cur];
+    return SWE_OK;
+}
+
+int swe_snapshot_begin(swe_mesh *m, double *h, double *hu, double *hv, double *t)
+{
+    if (!m || !h || !hu || !hv) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
+    int rc = snapshot_finish(m);
+    if (rc != SWE_OK) return rc;
+    if (!m->side) {
+        CK(cudaStreamCreateWithFlags(&m->side, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&m->ev_ready, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&m->ev_done, cudaEventDisableTiming));
+        CK(cudaHostAlloc((void **)&m->snap_ctrl, sizeof(Ctrl), cudaHostAllocDefault));
+    }
+    const size_t n = (size_t)m->T.nt;
+    double *st = m->d_stage;
+    // main stream: convert the current state into the staging buffer, then go on stepping
+    rc = swe_get_state_device(m, st, st + n, st + 2 * n);
+    if (rc != SWE_OK) return rc;
+    CK(cudaMemcpyAsync(m->snap_ctrl, m->P.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, m->stream));
+    CK(cudaEventRecord(m->ev_ready, m->stream));
+    // side stream: device -> host while the main stream runs the next steps
+    CK(cudaStreamWaitEvent(m->side, m->ev_ready, 0));
+    CK(cudaMemcpyAsync(h, st, n * sizeof(double), cudaMemcpyDeviceToHost, m->side));
+    CK(cudaMemcpyAsync(hu, st + n, n * sizeof(double), cudaMemcpyDeviceToHost, m->side));
+    CK(cudaMemcpyAsync(hv, st + 2 * n, n * sizeof(double), cudaMemcpyDeviceToHost, m->side));
+    CK(cudaEventRecord(m->ev_done, m->side));
+    m->snap_pending = true; m->snap_t = t; m->snap_cur = m->cur;
+    return SWE_OK;
+}
+
+int swe_snapshot_wait(swe_mesh *m)
+{
+    if (!m) return SWE_ERR_INVALID_ARG;
+    return snapshot_finish(m);
+}
+
 int swe_get_state(swe_mesh *m, double *h, double *hu, double *hv, double *t, double *dt_next)
 {
     if (!m) return SWE_ERR_INVALID_ARG;
@@ -645,7 +703,9 @@ int swe_get_state(swe_mesh *m, double *h, double *hu, double *hv, double *t, dou
     const size_t n = (size_t)m->T.nt;
     double *st = m->d_stage;
     if (h || hu || hv) {
-        int rc = swe_get_state_device(m, h ? st : nullptr, hu ? st + n : nullptr, hv ? st + 2 * n : nullptr);
+        int rc = snapshot_finish(m);
+        if (rc != SWE_OK) return rc;
+        rc = swe_get_state_device(m, h ? st : nullptr, hu ? st + n : nullptr, hv ? st + 2 * n : nullptr);
         if (rc != SWE_OK) return rc;
         if (h) CK(cudaMemcpyAsync(h, st, n * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
         if (hu) CK(cudaMemcpyAsync(hu, st + n, n * sizeof(double), cudaMemcpyDeviceToHost, m->stream));

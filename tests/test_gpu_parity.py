@@ -323,3 +323,28 @@ def test_zero_threshold_and_zero_steps():
     for a, b in zip(before[:3], after[:3]):
         np.testing.assert_array_equal(a, b)
     assert before[3] == after[3]
+
+
+def test_asynchronous_snapshot_on_a_side_stream():
+    """swe_snapshot_begin: the snapshot holds the state at the moment of the call although more
+    steps are queued right behind it, and it does not disturb them."""
+    import torch
+    w = W.config2(nx=600, ny=60)
+    ref = B.SweMesh.from_workload(w).bind_device()
+    ref.set_state(w.h, w.hu, w.hv)
+    ref.run(150)
+    mid = ref.get_state()
+    ref.run(250)
+    end = ref.get_state()
+    m = B.SweMesh.from_workload(w).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    bufs = [torch.empty(w.ncells, dtype=torch.float64).pin_memory().numpy() for _ in range(3)]
+    m.run(150)
+    m.snapshot_begin(*bufs)
+    m.run(250)                              # queued while the snapshot is being copied
+    t_snap = m.snapshot_wait()
+    for a, b in zip(bufs, mid[:3]):
+        np.testing.assert_array_equal(a, b)
+    assert t_snap == mid[3]
+    for a, b in zip(m.get_state()[:4], end[:4]):
+        np.testing.assert_array_equal(a, b)
