@@ -56,6 +56,9 @@ typedef enum {
 enum { SWE_BC_WALL = 1, SWE_BC_TRANSMISSIVE = 2, SWE_BC_INFLOW0 = 3, SWE_BC_MAX_TAG = 127 };
 /* swe_params.ordering: create-time renumbering of the cells for gather locality */
 enum { SWE_ORDER_IDENTITY = 0, SWE_ORDER_HILBERT = 1, SWE_ORDER_RCM = 2 };
+/* swe_params.riemann: HLLC (the paper's scheme) or plain HLL for all three
+ * components (eq.17-18) */
+enum { SWE_RIEMANN_HLLC = 0, SWE_RIEMANN_HLL = 1 };
 /* swe_params.loop_mode: how swe_run iterates without host round trips */
 enum { SWE_LOOP_AUTO = 0, SWE_LOOP_GRAPH = 1, SWE_LOOP_PERSISTENT = 2, SWE_LOOP_LAUNCH = 3 };
 
@@ -67,7 +70,7 @@ typedef struct {
     int32_t ordering;   /* SWE_ORDER_*; default SWE_ORDER_HILBERT */
     int32_t block_size; /* cells per tile = CUDA threads per block: 64, 128, 192 or 256; 0 = default (192) */
     int32_t loop_mode;  /* SWE_LOOP_*; default SWE_LOOP_AUTO */
-    int32_t reserved;   /* must be 0 */
+    int32_t riemann;    /* SWE_RIEMANN_*; default SWE_RIEMANN_HLLC */
 } swe_params;
 
 typedef struct {

@@ -17,6 +17,8 @@
  * Readings of silent / garbled passages are the R-numbers of DESIGN.md section 4.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"):
+ *   oracle_hll         : equals HLLC for equal tangential velocities; pure shear closed form
+ *                        -a h (v_R - v_L) / 2 (HLLC: 0); consistency
  *   oracle_hllc        : hand-computed single-edge values (tests/golden/), consistency
  *                        G(U,U) = physical flux, supercritical upwinding, antisymmetry
  *   geometry/neighbours: 2-triangle hand-computed update, rotation invariance
@@ -73,6 +75,7 @@ typedef struct {
     double *bstep;         /* [nb] G1 * L * dt of the current step */
     long double bvol_tag[MAX_TAGS]; /* cumulative outward volume per tag */
     int nthreads;
+    int hll;               /* 0: HLLC third component (eq.24), 1: plain HLL for all three (eq.17-18) */
 } oracle_mesh;
 
 /* ---------------------------------------------------------------------------------
@@ -83,7 +86,7 @@ typedef struct {
  * 1 left dry, 2 right dry, 3 rarefaction (eq.22), 4 shock (eq.23).
  * -------------------------------------------------------------------------------*/
 static void hllc(double g, double hdry, double hL, double uL, double vL, double hR, double uR,
-                 double vR, double G[3], double *diag)
+                 double vR, double G[3], double *diag, int hll)
 {
     double SL, SR, Ss, h0 = 0.0, hs = 0.0, pL = 1.0, pR = 1.0;
     int branch;
@@ -140,6 +143,10 @@ static void hllc(double g, double hdry, double hL, double uL, double vL, double 
     /* eq.(18); mass as printed, momentum in the algebraically identical difference form (R-12) */
     G[0] = ((SR * GL0 - SL * GR0) + SR * SL * (hR - hL)) / (SR - SL);
     G[1] = GL1 + SL * (SR * (hR * uR - hL * uL) - (GR1 - GL1)) / (SR - SL);
+    if (hll) { /* plain HLL: eq.(18) for the third component too */
+        G[2] = ((SR * GL2 - SL * GR2) + SR * SL * (hR * vR - hL * vL)) / (SR - SL);
+        return;
+    }
     /* eq.(24), R-16: tangential velocity upwinded by the sign of S* */
     G[2] = G[0] * (Ss >= 0.0 ? vL : vR);
 }
@@ -147,7 +154,13 @@ static void hllc(double g, double hdry, double hL, double uL, double vL, double 
 void oracle_hllc(double g, double hdry, double hL, double uL, double vL, double hR, double uR,
                  double vR, double *G, double *diag)
 {
-    hllc(g, hdry, hL, uL, vL, hR, uR, vR, G, diag);
+    hllc(g, hdry, hL, uL, vL, hR, uR, vR, G, diag, 0);
+}
+
+void oracle_hll(double g, double hdry, double hL, double uL, double vL, double hR, double uR,
+                double vR, double *G)
+{
+    hllc(g, hdry, hL, uL, vL, hR, uR, vR, G, NULL, 1);
 }
 
 /* ---------------------------------------------------------------------------------
@@ -293,6 +306,7 @@ int oracle_set_inflow(oracle_mesh *m, int tag, double Q_total)
 }
 
 void oracle_set_threads(oracle_mesh *m, int n) { m->nthreads = n > 0 ? n : 1; }
+void oracle_set_riemann(oracle_mesh *m, int hll) { m->hll = hll != 0; }
 int oracle_get_threads(const oracle_mesh *m) { return m->nthreads; }
 
 void oracle_set_state(oracle_mesh *m, const double *h, const double *hu, const double *hv, double t0)
@@ -354,7 +368,7 @@ static void step(oracle_mesh *m, double dt)
                 hL = hi + (zi - zf); if (hL < 0.0) hL = 0.0;
                 double hR = hj + (zj - zf); if (hR < 0.0) hR = 0.0;
                 const double uR = uj * n1 + vj * n2, vR = -uj * n2 + vj * n1;
-                hllc(g, hdry, hL, uL, vL, hR, uR, vR, G, NULL);
+                hllc(g, hdry, hL, uL, vL, hR, uR, vR, G, NULL, m->hll);
             } else { /* boundary edge */
                 const int tag = m->tag[3 * i + k];
                 hL = hi;

@@ -40,6 +40,8 @@ def lib():
         L.oracle_get_stats.argtypes = [C.c_void_p, dp]
         L.oracle_get_geometry.argtypes = [C.c_void_p, C.POINTER(C.c_int64), dp, dp, dp, dp, dp, dp]
         L.oracle_hllc.argtypes = [C.c_double] * 8 + [dp, dp]
+        L.oracle_hll.argtypes = [C.c_double] * 8 + [dp]
+        L.oracle_set_riemann.argtypes = [C.c_void_p, C.c_int]
         _lib = L
     return _lib
 
@@ -55,6 +57,13 @@ def hllc(hL, uL, vL, hR, uR, vR, g=9.81, h_dry=1e-6):
     lib().oracle_hllc(g, h_dry, hL, uL, vL, hR, uR, vR, _dp(G), _dp(d))
     names = ["branch", "h0", "hs", "pL", "pR", "SL", "SR", "Sstar"]
     return G, dict(zip(names, d.tolist()))
+
+
+def hll(hL, uL, vL, hR, uR, vR, g=9.81, h_dry=1e-6):
+    """Single-edge plain HLL flux (all three components by eq.17-18) in the edge frame."""
+    G = np.zeros(3)
+    lib().oracle_hll(g, h_dry, hL, uL, vL, hR, uR, vR, _dp(G))
+    return G
 
 
 class OracleSolver:
@@ -99,6 +108,10 @@ class OracleSolver:
     @property
     def threads(self):
         return self._L.oracle_get_threads(self._h)
+
+    def set_riemann(self, hll):
+        """hll=True: plain HLL instead of HLLC."""
+        self._L.oracle_set_riemann(self._h, int(bool(hll)))
 
     def set_threads(self, n):
         self._L.oracle_set_threads(self._h, int(n))

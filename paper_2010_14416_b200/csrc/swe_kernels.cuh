@@ -72,6 +72,7 @@ struct Params {
     double *pmax0, *pmax1;    // [npart] per-block max rate of state U0 / U1
     Ctrl *ctrl;
     int32_t nt, ntiles, npart, max_edges, max_halo;
+    int32_t hll;              // 1: plain HLL for the tangential momentum too (SWE_RIEMANN_HLL)
     double g, hg, inv_g, cfl, hdry;   // hg = g/2
     // selected with a ternary so the kernel parameter block is never indexed dynamically
     __host__ __device__ __forceinline__ Rec *U(int c) const { return c ? U1 : U0; }
@@ -166,7 +167,8 @@ __device__ __forceinline__ double reduce_dt(const Params &P, const double *pmax,
 __device__ __forceinline__ void hllc_flux(const double g, const double hg, const double inv_g,
                                           const double hdry, double hL, double uL, double vL,
                                           double hR, double uR, double vR, const double pL,
-                                          const double pR, double &G0, double &G1, double &G2)
+                                          const double pR, const bool hll, double &G0, double &G1,
+                                          double &G2)
 {
     const bool dL = hL <= hdry, dR = hR <= hdry;           // R-15
     G0 = 0.0; G1 = 0.0; G2 = 0.0;
@@ -215,6 +217,8 @@ __device__ __forceinline__ void hllc_flux(const double g, const double hg, const
     // of eq.(25) equals -(SR-SL) G0 and its denominator is negative, so sign(S*) = sign(G0);
     // in the dry-bed cases eq.(26) sets S* = SL (left dry) or SR (right dry), the same sign.
     G2 = G0 * (G0 >= 0.0 ? vL : vR);
+    // plain HLL: eq.(18) for the third component too
+    if (hll) G2 = ((SR * (qL * vL) - SL * (qR * vR)) + SR * SL * (hR * vR - hL * vL)) * inv;
 }
 
 // ---- one edge: a2-a7 of SURVEY.md section 8(a) -------------------------------------------------
@@ -237,7 +241,7 @@ __device__ __forceinline__ void edge_eval(const Params &P, const EdgeRec &er, co
         const double hR = fmax(0.0, B.h + (B.z - zf));
         const double uR = fma(B.u, n1, B.v * n2), vR = fma(B.v, n1, -(B.u * n2));
         const double hL2 = hL * hL, hR2 = hR * hR;
-        hllc_flux(g, hg, P.inv_g, hdry, hL, uL, vL, hR, uR, vR, hg * hL2, hg * hR2, G0, G1, G2);
+        hllc_flux(g, hg, P.inv_g, hdry, hL, uL, vL, hR, uR, vR, hg * hL2, hg * hR2, P.hll != 0, G0, G1, G2);
         // bathymetry source eq.(30) with g/2 (R-13), one value per side
         sba = hg * (hL2 - A.h * A.h);
         sbb = hg * (hR2 - B.h * B.h);

@@ -210,7 +210,7 @@ int swe_params_default(swe_params *p)
 {
     if (!p) return SWE_ERR_INVALID_ARG;
     p->g = 9.81; p->cfl = 0.9; p->h_dry = 1e-6;
-    p->ordering = SWE_ORDER_HILBERT; p->block_size = 0; p->loop_mode = SWE_LOOP_AUTO; p->reserved = 0;
+    p->ordering = SWE_ORDER_HILBERT; p->block_size = 0; p->loop_mode = SWE_LOOP_AUTO; p->riemann = SWE_RIEMANN_HLLC;
     return SWE_OK;
 }
 
@@ -230,7 +230,7 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     swe_params_default(&p);
     if (params) p = *params;
     if (!(p.g > 0.0) || !(p.cfl > 0.0) || !(p.h_dry >= 0.0) || p.ordering < 0 || p.ordering > SWE_ORDER_RCM ||
-        p.loop_mode < 0 || p.loop_mode > SWE_LOOP_LAUNCH ||
+        p.loop_mode < 0 || p.loop_mode > SWE_LOOP_LAUNCH || p.riemann < 0 || p.riemann > SWE_RIEMANN_HLL ||
         (p.block_size != 0 && p.block_size != 64 && p.block_size != 128 && p.block_size != 192 && p.block_size != 256)) {
         g_create_err = "swe_mesh_create: invalid swe_params (block_size must be 0, 64, 128, 192 or 256)";
         return SWE_ERR_INVALID_ARG;
@@ -389,6 +389,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
     m->d_qn = (double *)(m->ws + L.qn); P.qn_tag = m->d_qn;
     P.ctrl = (Ctrl *)(m->ws + L.ctrl);
+    P.hll = m->prm.riemann == SWE_RIEMANN_HLL;
     P.nt = (int32_t)T.nt; P.ntiles = ntiles; P.max_edges = X.max_edges; P.max_halo = X.max_halo;
     P.npart = mode == SWE_LOOP_PERSISTENT ? m->coop_grid : m->grid;
     P.g = m->prm.g; P.hg = 0.5 * m->prm.g; P.inv_g = 1.0 / m->prm.g; P.cfl = m->prm.cfl;

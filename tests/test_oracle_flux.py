@@ -144,3 +144,35 @@ def test_stoker_golden_digits():
                               (e["hm"], e["um"], e["shock"], e["head"], e["tail"])):
             assert have == pytest.approx(want, rel=1e-11)
     assert rows["ritter_1"][4] == pytest.approx(2 * math.sqrt(G), rel=1e-12)
+
+
+# ------------------------------------------------------------------ plain HLL
+def test_hll_equals_hllc_for_equal_tangential_velocity():
+    """eq.(18) on the third component with v_L = v_R = v gives v times the HLL mass flux, which is
+    what eq.(24) gives too; components 1-2 are shared by construction."""
+    from oracle.swe_oracle import hll
+    for (hL, uL, hR, uR, v) in [(1.0, 0.0, 0.5, 0.0, 0.3), (1.0, -1.0, 1.0, 1.0, -0.7),
+                                (0.8, 0.4, 1.3, -0.2, 2.0), (1.0, 0.5, 0.0, 0.0, 0.25)]:
+        Gc, _ = hllc(hL, uL, v, hR, uR, v)
+        Gh = hll(hL, uL, v, hR, uR, v)
+        np.testing.assert_allclose(Gh, Gc, rtol=1e-14, atol=1e-15)
+
+
+def test_hll_pure_shear_closed_form():
+    """Equal depths at rest in the normal direction, tangential velocities v_L != v_R: S_L = -a,
+    S_R = a, so eq.(18) gives G_3 = S_R S_L h (v_R - v_L) / (S_R - S_L) = -a h (v_R - v_L) / 2, the
+    numerical diffusion of a contact that HLLC removes (its G_3 is G_1 v = 0)."""
+    from oracle.swe_oracle import hll
+    h, vL, vR = 0.9, 0.4, -1.1
+    a = (9.81 * h) ** 0.5
+    Gh = hll(h, 0.0, vL, h, 0.0, vR)
+    assert Gh[0] == 0.0 and Gh[1] == pytest.approx(0.5 * 9.81 * h * h, rel=1e-15)
+    assert Gh[2] == pytest.approx(-a * h * (vR - vL) / 2.0, rel=1e-14)
+    Gc, _ = hllc(h, 0.0, vL, h, 0.0, vR)
+    assert Gc[2] == 0.0
+
+
+def test_hll_consistency_and_supercritical():
+    from oracle.swe_oracle import hll
+    for (h, u, v) in [(0.7, 0.3, -0.2), (0.2, 3.0, 1.0), (0.2, -3.0, 1.0)]:
+        np.testing.assert_allclose(hll(h, u, v, h, u, v), _phys(h, u, v), rtol=1e-14, atol=1e-15)
