@@ -362,9 +362,11 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     // dynamic shared memory of the tile pipeline (swe_kernels.cuh), sized for this mesh's longest lists
     const TileTables &X = m->X;
     m->smem = tile_smem_bytes(m->block, X.max_halo, X.max_edges);
-    if (m->smem > (size_t)smem_optin) { m->err = "tile does not fit in shared memory"; return SWE_ERR_CUDA; }
+    if (m->smem > (size_t)smem_optin - 1024) { m->err = "tile does not fit in shared memory"; return SWE_ERR_CUDA; }
     m->kern = step_kernel_for(m->block);
-    CK(cudaFuncSetAttribute((const void *)m->kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem));
+    // the attribute belongs to the kernel, not to this handle: allow the device maximum so that
+    // handles with different tile tables can coexist
+    CK(cudaFuncSetAttribute((const void *)m->kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 1024));
     int occ_step = 0, occ_pers = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_step, (const void *)m->kern, m->block, m->smem));
     occ_pers = occ_step;

@@ -365,3 +365,21 @@ def test_plain_hll_solver_matches_oracle():
     c.set_state(w.h, w.hu, w.hv)
     c.run(600)
     assert np.abs(c.get_state()[0] - hg).max() > 1e-6
+
+
+def test_two_handles_with_different_shared_memory_needs_interleave():
+    """Handles whose tile tables need different amounts of shared memory (random numbering: 3 x the
+    edges and halo) keep working when their runs alternate."""
+    w = W.config5("0.1M", nsteps=60)
+    a = B.SweMesh.from_workload(w, ordering=B.ORDER_IDENTITY, loop_mode=B.LOOP_GRAPH).bind_device()
+    b = B.SweMesh.from_workload(w, ordering=B.ORDER_HILBERT, loop_mode=B.LOOP_GRAPH).bind_device()
+    assert a.get_tile_info()["smem_bytes"] > 1.5 * b.get_tile_info()["smem_bytes"]
+    for m in (a, b):
+        m.set_state(w.h, w.hu, w.hv)
+    for _ in range(3):
+        a.run(10)
+        b.run(10)
+        b.run(10)
+        a.run(10)
+    for x, y in zip(a.get_state()[:4], b.get_state()[:4]):
+        np.testing.assert_array_equal(x, y)
