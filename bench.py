@@ -70,12 +70,17 @@ def load_peaks():
 
 
 def load_traffic(workload: str):
-    """dram bytes per launch of the step kernel from the committed ncu --set full capture."""
+    """dram bytes per launch of the step kernel from the committed ncu --set full capture
+    (profiles/traffic.csv: workload,dram_bytes_per_launch; profiles/r01_v8_README.md says how)."""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(workload)
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for line in f.read().splitlines()[1:]:
+                name, val = line.split(",")
+                if name == workload:
+                    return int(val)
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
