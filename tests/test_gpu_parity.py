@@ -383,3 +383,23 @@ def test_two_handles_with_different_shared_memory_needs_interleave():
         a.run(10)
     for x, y in zip(a.get_state()[:4], b.get_state()[:4]):
         np.testing.assert_array_equal(x, y)
+
+
+def test_non_default_parameters_two_inflow_groups_rcm():
+    """g, CFL and h_dry away from their defaults, two prescribed-discharge groups (one of them an
+    extraction, Q < 0), RCM ordering, persistent loop: every table and constant that carries a
+    parameter is exercised against the oracle."""
+    w = W.config4(nx=240, ny=60)
+    w.g, w.cfl, w.h_dry = 3.71, 0.45, 2e-4            # Mars gravity, cautious CFL, coarse threshold
+    # second group: the wet cells of the right edge pump water out instead of draining freely
+    tags = w.bc_tags.copy()
+    tags[tags == W.BC_TRANSMISSIVE] = W.BC_INFLOW0 + 1
+    w.bc_tags = tags
+    w.bc_values = {W.BC_INFLOW0: 350.0, W.BC_INFLOW0 + 1: -40.0}
+    m, o = run_both(w, 800, ordering=B.ORDER_RCM, loop_mode=B.LOOP_PERSISTENT)
+    assert_parity(m, o, w)
+    vg, vo = m.get_boundary_volumes(), o.boundary_volumes()
+    np.testing.assert_allclose(vg, vo, rtol=1e-10, atol=1e-10)
+    t = m.get_state()[3]
+    assert vg[W.BC_INFLOW0] == pytest.approx(-350.0 * t, rel=1e-12)
+    assert vg[W.BC_INFLOW0 + 1] == pytest.approx(40.0 * t, rel=1e-12)
