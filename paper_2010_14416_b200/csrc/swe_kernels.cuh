@@ -69,6 +69,8 @@ struct Params {
     const int32_t *tinfo;     // [ntiles][4 + max_halo] per-tile info block, see "the tile pipeline"
     const double *qn_tag;     // [128] unit discharge along the outward normal per inflow tag
     double *bvol;             // [boundary edges] cumulative outward volume through each boundary edge
+    int4 *hint;               // [ntiles] .x = 1 if the tile was active (not all dry) at the previous step
+                              // (16-byte entries: fetched with cp.async.cg, which bypasses L1)
     double *pmax0, *pmax1;    // [npart] per-block max rate of state U0 / U1
     Ctrl *ctrl;
     int32_t nt, ntiles, npart, max_edges, max_halo;
@@ -376,6 +378,8 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 //   double  scell[3][TC]           1/|Omega|, 1/R, g m^2
 //   int32   sinfo[3][4 + MH]       info blocks (three tiles deep)
 //   uint64  bar[7]                 rec[2], info[3], edge[2]
+//   int32   eflag[2]               was the edge list of the tile in stage s requested?
+//   int4    shint[4]               P.hint entries of the next tiles (cp.async by the producer thread)
 // Schedule for the block's n-th tile (s = n & 1), all copies asynchronous and one tile ahead
 // (measured: with the edge list issued only after the edge phase, blocks spent 26 % of their
 // time waiting for it):
@@ -394,7 +398,7 @@ __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int M
 {
     return ((size_t)TC * 9 + 28) * sizeof(double) + 2 * (size_t)(TC + MH) * sizeof(Rec) +
            2 * (size_t)ME * sizeof(EdgeRec) + (size_t)TC * 3 * sizeof(double) +
-           3 * (size_t)(kInfoHdr + MH) * sizeof(int32_t) + kNumBars * sizeof(uint64_t);
+           3 * (size_t)(kInfoHdr + MH) * sizeof(int32_t) + kNumBars * sizeof(uint64_t) + 32 + 4 * sizeof(int4);
 }
 template <int TC> struct TilePipe {
     double *so; Rec *srec0; EdgeRec *sedge0; double *scell; int32_t *sinfo0; uint64_t *bar;
@@ -406,6 +410,12 @@ template <int TC> struct TilePipe {
     __device__ __forceinline__ uint64_t *rbar(int s) const { return bar + s; }
     __device__ __forceinline__ uint64_t *ibar(int j) const { return bar + 2 + j; }
     __device__ __forceinline__ uint64_t *ebar(int s) const { return bar + 5 + s; }
+    // eflag[s]: bit 0 = an edge-list copy into sedge[s] was issued for the tile that uses stage s,
+    // bit 1 = parity to wait for on ebar(s); ecnt[s] (producer only) = completed copies into stage s
+    __device__ __forceinline__ volatile int32_t *eflag() const { return reinterpret_cast<volatile int32_t *>(bar + kNumBars); }
+    // ring of hints fetched ahead by the producer thread
+    __device__ __forceinline__ volatile int32_t *ecnt() const { return reinterpret_cast<volatile int32_t *>(bar + kNumBars) + 2; }
+    __device__ __forceinline__ int4 *shint(unsigned m) const { return reinterpret_cast<int4 *>(bar + kNumBars + 3) + (m & 3u); }
 };
 template <int TC> __device__ __forceinline__ TilePipe<TC> make_pipe(const Params &P, unsigned char *smem)
 {
@@ -457,17 +467,22 @@ template <int TC> __device__ __forceinline__ void gather_halo(const TilePipe<TC>
     }
 }
 
-// All the tiles of this block for one time step.  `n0` = number of tiles this block has pushed
-// through the pipeline before (persistent loop), which fixes the buffers and barrier parities.
+// Pipeline state carried across the steps of a persistent launch: tiles pushed through so far
+// (fixes buffers and barrier parities).  The edge barriers complete a phase only when a list was
+// requested, so their parity is kept by the producer thread in shared memory (ecnt) and published
+// with the request flag: eflag[s] = requested | parity << 1.
+struct PipeState { unsigned n = 0; };
+
+// All the tiles of this block for one time step.
 // Returns this thread's maximum rate contribution.
 template <int TC>
 __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC> &pp,
                                              const Rec *__restrict__ Uin, Rec *__restrict__ Uout,
-                                             const double dt, unsigned &nclamp, unsigned &n0)
+                                             const double dt, unsigned &nclamp, PipeState &ps)
 {
     const int tid = threadIdx.x, G = gridDim.x;
     double rate = 0.0;
-    unsigned n = n0;
+    unsigned n = ps.n;
     int tile = blockIdx.x;
     if (tile >= P.ntiles) return 0.0;
     // ---- prologue: everything tile n needs, and the info block of tile n+1
@@ -475,12 +490,20 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
     // iteration than the last ones (ne ~ 1.66 TC), so the last warp has the slack (measured: with
     // thread 0 as producer warp 0 reached the mid barrier ~1000 cycles late)
     const bool producer = tid == TC - 32;
+    // Edge lists are 40 of the ~105 bytes a cell costs and an all-dry tile never reads its list, so
+    // the list of the NEXT tile is requested only if that tile was active at the previous step
+    // (P.hint, read one tile early); a tile that turns out active without its list (the wet front
+    // reached it) fetches it on the spot.
     if (producer) {
         issue_info(P, pp, tile, n % 3);
         issue_recs(P, pp, Uin, tile, n & 1);
         const int32_t *gi = P.tinfo + (size_t)tile * pp.info_stride;
-        issue_edges(P, pp, __ldg(gi), __ldg(gi + 1), n & 1);
-        if (tile + G < P.ntiles) issue_info(P, pp, tile + G, (n + 1) % 3);
+        issue_edges(P, pp, __ldg(gi), __ldg(gi + 1), n & 1);      // the step's first tile: always
+        pp.eflag()[n & 1] = 1 | ((pp.ecnt()[n & 1] & 1) << 1);
+        if (tile + G < P.ntiles) {
+            issue_info(P, pp, tile + G, (n + 1) % 3);
+            cp_async16(pp.shint(n + 1), P.hint + tile + G);           // lands before the first barrier
+        }
     }
     mbar_wait(pp.ibar(n % 3), (n / 3) & 1u);
     gather_halo(pp, Uin, n % 3, n & 1);
@@ -493,7 +516,6 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
         // ---- top
         cp_async_wait<0>();                               // own halo gathers of this tile
         mbar_wait(pp.rbar(s), (n >> 1) & 1u);
-        mbar_wait(pp.ebar(s), (n >> 1) & 1u);
         const Rec *const srec = pp.srec(s);
         const EdgeRec *const sedge = pp.sedge(s);
         const int32_t *const info = pp.sinfo(n % 3);
@@ -520,12 +542,29 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
         if (have_next) {
             mbar_wait(pp.ibar((n + 1) % 3), ((n + 1) / 3) & 1u);
             if (producer) {
-                const int32_t *ni = pp.sinfo((n + 1) % 3);
-                issue_edges(P, pp, ni[0], ni[1], s ^ 1);
+                const int hint_next = pp.shint(n + 1)->x;            // requested one tile ago
+                pp.eflag()[s ^ 1] = (hint_next != 0) | ((pp.ecnt()[s ^ 1] & 1) << 1);
+                if (hint_next) {
+                    const int32_t *ni = pp.sinfo((n + 1) % 3);
+                    issue_edges(P, pp, ni[0], ni[1], s ^ 1);
+                }
+                if (tile + 2 * G < P.ntiles) cp_async16(pp.shint(n + 2), P.hint + tile + 2 * G);
             }
             gather_halo(pp, Uin, (n + 1) % 3, s ^ 1);
         }
         cp_async_commit();
+        if (producer) P.hint[tile].x = active;
+        // this tile's edge list: requested one tile ago (flag written before the barrier above),
+        // or fetched now if the tile is active without it
+        {
+            const int f = pp.eflag()[s];
+            const bool requested = (f & 1) != 0;
+            if (!requested && active && producer) issue_edges(P, pp, info[0], ne, s);
+            if (requested || active) {
+                mbar_wait(pp.ebar(s), (unsigned)f >> 1);
+                if (producer) pp.ecnt()[s] = pp.ecnt()[s] + 1;
+            }
+        }
         if (!active) {
             // Every cell of the tile and every neighbour is dry and no discharge is prescribed:
             // all fluxes vanish, h' = h + 0, and dry cells carry u = v = 0 already (R-15), so the
@@ -570,7 +609,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
         }
     }
     cp_async_wait<0>();
-    n0 = n;
+    ps.n = n;
     return rate;
 }
 

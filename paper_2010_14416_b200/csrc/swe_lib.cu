@@ -43,10 +43,11 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
     const TilePipe<TC> pp = make_pipe<TC>(P, dyn_smem);
     if (threadIdx.x == 0) {
         for (int s = 0; s < kNumBars; s++) mbar_init(pp.bar + s, 1);
+        pp.ecnt()[0] = 0; pp.ecnt()[1] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    unsigned it = 0;
+    PipeState it;
     for (long long s = 0; s < nsteps; s++) {
         const double dt_cfl = reduce_dt(P, P.pmax(cur), s_red);
         // swe_run_until: the step that would pass t_end ends on it; after that, zero steps
@@ -185,7 +186,7 @@ static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 namespace {
 static_assert(sizeof(HostEdge) == sizeof(EdgeRec) && kHostIdBits == kIdBits, "table records");
 struct Layout {
-    size_t U0, U1, cellc, edges, tinfo, bvol, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
+    size_t U0, U1, cellc, edges, tinfo, bvol, hint, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
 };
 Layout make_layout(const HostTables &T, const TileTables &X)
 {
@@ -195,6 +196,7 @@ Layout make_layout(const HostTables &T, const TileTables &X)
     L.cellc = take(X.cellc.size() * sizeof(double)); L.edges = take(X.edges.size() * sizeof(EdgeRec));
     L.tinfo = take(X.tinfo.size() * sizeof(int32_t));
     L.bvol = take(((size_t)X.nbedges + 1) * sizeof(double));
+    L.hint = take(((size_t)X.ntiles + 1) * sizeof(int4));
     L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
     L.stage = take(3 * n * sizeof(double));
     L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
@@ -386,6 +388,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.cellc = (const double *)(m->ws + L.cellc); P.edges = (const EdgeRec *)(m->ws + L.edges);
     P.tinfo = (const int32_t *)(m->ws + L.tinfo);
     P.bvol = (double *)(m->ws + L.bvol);
+    P.hint = (int4 *)(m->ws + L.hint);
     m->d_zcell = (double *)(m->ws + L.zcell); m->d_inv = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
@@ -441,6 +444,7 @@ static int set_state_common(swe_mesh *m, const double *h, const double *hu, cons
     m->cur = 0;
     m->have_state = false; m->have_rates = false;
     Ctrl c{}; c.t[0] = t0; c.t[1] = t0; c.t_end = INFINITY; c.bad_cell = INT32_MAX;
+    CK(cudaMemsetAsync(m->P.hint, 1, (size_t)m->X.ntiles * sizeof(int4), m->stream));   // nothing known yet: every tile active (.x != 0)
     if (m->X.nbedges > 0) CK(cudaMemsetAsync(m->P.bvol, 0, (size_t)m->X.nbedges * sizeof(double), m->stream));
     CK(cudaMemcpyAsync(m->P.ctrl, &c, sizeof(Ctrl), cudaMemcpyHostToDevice, m->stream));
     swe_pack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_inv, h, hu, hv, m->d_zcell);
