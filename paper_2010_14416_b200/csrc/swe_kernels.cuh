@@ -1,12 +1,15 @@
 // Device code of libswe_b200: the fused, tiled, edge-once SWE step for sm_100a (FP64).
 //
 // The cells are numbered along a space-filling curve (mesh_builder.cpp) and cut into tiles of
-// blockDim.x consecutive cells.  A thread block walks tiles through a two-stage pipeline:
+// blockDim.x consecutive cells.  A thread block walks tiles through a software pipeline:
 //
-//   stage    one elected thread issues three TMA bulk copies (cp.async.bulk, mbarrier
-//            complete_tx) for the tile's three CONTIGUOUS streams: the state records of its
-//            cells, its edge list and its cell constants.  The copies for tile n+1 are in
-//            flight while tile n is computed; nothing passes through registers.
+//   stage    one elected thread issues TMA bulk copies (cp.async.bulk, mbarrier complete_tx)
+//            for the tile's CONTIGUOUS streams: the state records of its cells, its edge list,
+//            its info block (halo ids).  The copies for tile n+1 are in flight while tile n is
+//            computed; nothing passes through registers.  Halo records and cell constants come
+//            by per-thread cp.async.  A tile whose cells and halo are all dry (and that has no
+//            inflow edge) copies its records and skips everything else; the edge list of a tile
+//            that was like that at the previous step is not even requested.
 //   phase 1  (edge-parallel) every edge that touches the tile is evaluated ONCE: hydrostatic
 //            reconstruction, rotation, HLLC flux, rotation back, both sides' bathymetry source;
 //            the signed, length-weighted result goes to the (cell, local edge) slots of its end
