@@ -59,7 +59,9 @@ enum { SWE_ORDER_IDENTITY = 0, SWE_ORDER_HILBERT = 1, SWE_ORDER_RCM = 2 };
 /* swe_params.riemann: HLLC (the paper's scheme) or plain HLL for all three
  * components (eq.17-18) */
 enum { SWE_RIEMANN_HLLC = 0, SWE_RIEMANN_HLL = 1 };
-/* swe_params.loop_mode: how swe_run iterates without host round trips */
+/* swe_params.loop_mode: how swe_run iterates without host round trips: GRAPH = CUDA graphs of
+ * 128 / 16 / 2 step-kernel launches, PERSISTENT = one cooperative launch with a grid barrier per
+ * step, LAUNCH = plain launches; AUTO = GRAPH (measured as fast or faster at every mesh size) */
 enum { SWE_LOOP_AUTO = 0, SWE_LOOP_GRAPH = 1, SWE_LOOP_PERSISTENT = 2, SWE_LOOP_LAUNCH = 3 };
 
 typedef struct {
