@@ -31,7 +31,7 @@ if ROOT not in sys.path:
 from paper_2010_14416_b200 import workloads as W  # noqa: E402
 
 ALGO_BYTES_PER_CELL = 156.0   # 132 B read + 24 B written per cell-update
-METRIC = "SWE FP64 cell-updates/s"
+METRIC = "SWE FP64 cell-updates/s on 1 B200; achieved HBM GB/s vs peak"   # BASELINE.json "metric"
 UNIT = "cell-updates/s"
 
 
