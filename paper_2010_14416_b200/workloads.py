@@ -279,6 +279,38 @@ def config5(size: str, **kw) -> Workload:
 
 
 # ----------------------------------------------------------------------------------
+# locally refined mesh (the paper refines its river meshes around
+# bridge piers)
+# ----------------------------------------------------------------------------------
+def refined_basin(nx=240, ny=120, *, a=0.85, seed=20101 + 6, length=240.0, manning=0.03,
+                  nsteps=800) -> Workload:
+    """Walled basin whose cell size varies 12:1 (a = 0.85): the jittered triangulation is mapped by
+    x' = x + a L/(2 pi) sin(2 pi x / L) (and the same in y), which is monotone for a < 1, so the
+    smallest cells sit around the domain centre like a refinement patch.  Two Gaussian bumps on
+    the bed, a column of water released next to the fine region, Manning friction."""
+    rng = np.random.default_rng(seed)
+    dx = length / nx
+    xy, tris, ij = jittered_triangulation(nx, ny, dx, rng)
+    Lx, Ly = nx * dx, ny * dx
+    two_pi = 2.0 * np.pi
+    xy = np.stack([xy[:, 0] + a * Lx / two_pi * np.sin(two_pi * xy[:, 0] / Lx + np.pi),
+                   xy[:, 1] + a * Ly / two_pi * np.sin(two_pi * xy[:, 1] / Ly + np.pi)], 1)
+    tags = box_boundary_tags(tris, ij, nx, ny)
+    z = 0.4 * np.exp(-((xy[:, 0] - 0.35 * Lx) ** 2 + (xy[:, 1] - 0.6 * Ly) ** 2) / (2 * (0.06 * Lx) ** 2)) \
+        + 0.9 * np.exp(-((xy[:, 0] - 0.7 * Lx) ** 2 + (xy[:, 1] - 0.4 * Ly) ** 2) / (2 * (0.05 * Lx) ** 2))
+    c = centroids(xy, tris)
+    zc = cell_mean(z, tris)
+    r2 = (c[:, 0] - 0.45 * Lx) ** 2 + (c[:, 1] - 0.5 * Ly) ** 2
+    stage = np.where(r2 < (0.12 * Lx) ** 2, 1.6, 0.5)
+    h = np.maximum(0.0, stage - zc)
+    nt = tris.shape[0]
+    return Workload(name="refined_basin", nodes_xy=np.ascontiguousarray(xy), tris=tris, bathymetry=z,
+                    manning=np.full(nt, float(manning)), bc_tags=tags, h=h, hu=np.zeros(nt),
+                    hv=np.zeros(nt), cfl=0.9, nsteps=nsteps,
+                    meta=dict(nx=nx, ny=ny, dx=dx, a=a, seed=seed))
+
+
+# ----------------------------------------------------------------------------------
 # small meshes for unit tests
 # ----------------------------------------------------------------------------------
 def two_triangles(h_lower=1.0, h_upper=0.5) -> Workload:

@@ -403,3 +403,24 @@ def test_non_default_parameters_two_inflow_groups_rcm():
     t = m.get_state()[3]
     assert vg[W.BC_INFLOW0] == pytest.approx(-350.0 * t, rel=1e-12)
     assert vg[W.BC_INFLOW0 + 1] == pytest.approx(40.0 * t, rel=1e-12)
+
+
+def test_locally_refined_mesh():
+    """SURVEY.md section 8(f) NEXT-3 (second half): a mesh whose inradius varies 32:1 (the paper refines
+    around bridge piers).  The time step is set by the few smallest cells, tiles
+    cover very different areas, and the Hilbert order still keeps 90 % of the edges inside tiles."""
+    w = W.refined_basin()
+    m, o = run_both(w, w.nsteps)
+    assert_parity(m, o, w)
+    geo = o.geometry()
+    assert geo["rin"].max() / geo["rin"].min() > 25.0
+    assert m.get_tile_info()["edges_per_cell"] < 1.75
+    # dt is a min over cells of very different size: it must equal the oracle's to 1e-12 at every
+    # stage of the run, not only at the end
+    m2 = B.SweMesh.from_workload(w).bind_device()
+    m2.set_state(w.h, w.hu, w.hv)
+    o2 = OracleSolver.from_workload(w)
+    for _ in range(6):
+        assert m2.compute_dt() == pytest.approx(o2.compute_dt(), rel=1e-12)
+        m2.run(37)
+        o2.run(37)

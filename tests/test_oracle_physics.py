@@ -284,3 +284,18 @@ def test_boundary_volumes_per_tag_and_run_until():
     for a, b in zip(r.get_state()[:4], r2.get_state()[:4]):
         np.testing.assert_array_equal(a, b)
     assert r.get_state()[3] < 30.0 <= r.get_state()[3] + r.get_state()[4]
+
+
+def test_refined_mesh_mass_and_dt_scale():
+    """Locally refined basin (inradius ratio > 25): mass is conserved to round-off in the closed
+    box, and the CFL step is bounded by the smallest wet cell's R / sqrt(g h) (eq.15, R-9)."""
+    w = W.refined_basin(nx=120, ny=60)
+    s = OracleSolver.from_workload(w)
+    v0 = s.stats()["volume"]
+    geo = s.geometry()
+    wet = w.h > w.h_dry
+    bound = 0.9 * (geo["rin"][wet] / np.sqrt(G * w.h[wet])).min()
+    assert s.compute_dt() == pytest.approx(bound, rel=1e-14)       # at rest: lambda = sqrt(g h)
+    s.run(300)
+    assert s.stats()["volume"] == pytest.approx(v0, rel=1e-12)
+    assert s.stats()["nclamp"] == 0
