@@ -224,6 +224,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         m.run(args.steps)                          # call will replay (graphs are keyed by buffer parity)
     m.sync()
     launches0 = m.get_launch_info()["kernel_launches"]
+    active0 = m.get_stats()["active_tile_steps"]
     sampler = ClockSampler(local_rank)
     sampler.start()
     time.sleep(0.25)
@@ -241,6 +242,8 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     tiles = m.get_tile_info()
     launches = info["kernel_launches"] - launches0
     stats = m.get_stats()
+    # share of (tile, step) pairs that were not all dry: all-dry tiles copy their records (64 B/cell)
+    active_share = (stats["active_tile_steps"] - active0) / float(tiles["ntiles"] * args.steps)
 
     # ---- end-to-end leg through the C ABI with host buffers: set_state + run(K) + get_state ----
     barrier()
@@ -281,6 +284,13 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                    "n_clamped": stats["n_clamped"]},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic,
+                     # the same with 64 B (record in + out) for the cells of all-dry tiles, whose update
+                     # is the identity, and 156 B for the others
+                     "active_tile_share": active_share,
+                     "achieved_state_aware": (ALGO_BYTES_PER_CELL * active_share + 64.0 * (1.0 - active_share))
+                     * n / (kernel_ms * 1e-3) / 1e9,
+                     "frac_state_aware": (ALGO_BYTES_PER_CELL * active_share + 64.0 * (1.0 - active_share))
+                     * n / (kernel_ms * 1e-3) / 1e9 / peak,
                      "achieved_dram": None if traffic is None else traffic / (kernel_ms * 1e-3) / 1e9,
                      "frac_dram": None if traffic is None else traffic / (kernel_ms * 1e-3) / 1e9 / peak,
                      "kernel": f"swe_step_kernel<{tiles['tile_cells']}>", "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,

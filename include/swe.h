@@ -83,6 +83,9 @@ typedef struct {
     int64_t n_dry;        /* cells with h <= h_dry */
     int64_t n_clamped;    /* times a negative depth was clamped to 0 (R-15; expected 0) */
     int64_t n_nonfinite;  /* cells whose state is NaN/inf (expected 0) */
+    int64_t active_tile_steps; /* sum over the steps since swe_set_state of the number of tiles that were
+                                  not all dry (tile + halo dry, no inflow edge: such tiles copy their
+                                  records and skip the arithmetic) */
 } swe_stats;
 
 /* Fills *p with the defaults listed above. */

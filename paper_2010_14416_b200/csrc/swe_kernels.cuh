@@ -61,6 +61,7 @@ struct Ctrl {                 // device-resident loop state
     double t_end;             // the step that would pass t_end ends on it (swe_run_until); +inf otherwise
     long long steps;
     unsigned long long n_clamped;
+    unsigned long long n_active;  // tiles that were not all dry, summed over the steps (diagnostics)
     int all_dry;              // set when a step found no wet cell
     int bad_cell;             // smallest caller id with a negative depth or a non-finite value (swe_set_state)
 };
@@ -418,6 +419,8 @@ template <int TC> struct TilePipe {
     __device__ __forceinline__ volatile int32_t *eflag() const { return reinterpret_cast<volatile int32_t *>(bar + kNumBars); }
     // ring of hints fetched ahead by the producer thread
     __device__ __forceinline__ volatile int32_t *ecnt() const { return reinterpret_cast<volatile int32_t *>(bar + kNumBars) + 2; }
+    // nact (producer only): active tiles of this block in the current step
+    __device__ __forceinline__ volatile int32_t *nact() const { return reinterpret_cast<volatile int32_t *>(bar + kNumBars) + 4; }
     __device__ __forceinline__ int4 *shint(unsigned m) const { return reinterpret_cast<int4 *>(bar + kNumBars + 3) + (m & 3u); }
 };
 template <int TC> __device__ __forceinline__ TilePipe<TC> make_pipe(const Params &P, unsigned char *smem)
@@ -556,7 +559,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, const TilePipe<TC>
             gather_halo(pp, Uin, (n + 1) % 3, s ^ 1);
         }
         cp_async_commit();
-        if (producer) P.hint[tile].x = active;
+        if (producer) { P.hint[tile].x = active; if (active) *pp.nact() = *pp.nact() + 1; }
         // this tile's edge list: requested one tile ago (flag written before the barrier above),
         // or fetched now if the tile is active without it
         {

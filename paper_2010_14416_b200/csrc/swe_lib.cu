@@ -43,7 +43,7 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
     const TilePipe<TC> pp = make_pipe<TC>(P, dyn_smem);
     if (threadIdx.x == 0) {
         for (int s = 0; s < kNumBars; s++) mbar_init(pp.bar + s, 1);
-        pp.ecnt()[0] = 0; pp.ecnt()[1] = 0;
+        pp.ecnt()[0] = 0; pp.ecnt()[1] = 0; *pp.nact() = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -57,6 +57,10 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
         double rate = step_tiles<TC>(P, pp, P.U(cur), P.U(cur ^ 1), dt, nclamp, it);
         rate = block_max(rate, s_red);
         if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
+        if (threadIdx.x == TC - 32 && *pp.nact()) {                               // likewise
+            atomicAdd(&P.ctrl->n_active, (unsigned long long)*pp.nact());
+            *pp.nact() = 0;
+        }
         if (threadIdx.x == 0) {
             P.pmax(cur ^ 1)[blockIdx.x] = rate;
             if (blockIdx.x == 0) {
@@ -749,6 +753,7 @@ int swe_get_stats(swe_mesh *m, swe_stats *s)
     }
     s->volume = (double)vol; s->t = c.t[m->cur]; s->dt_last = c.dt_last; s->steps = c.steps;
     s->n_dry = ndry; s->n_clamped = (int64_t)c.n_clamped; s->n_nonfinite = nbad;
+    s->active_tile_steps = (int64_t)c.n_active;
     return SWE_OK;
 }
 

@@ -424,3 +424,22 @@ def test_locally_refined_mesh():
         assert m2.compute_dt() == pytest.approx(o2.compute_dt(), rel=1e-12)
         m2.run(37)
         o2.run(37)
+
+
+def test_active_tile_counter():
+    """swe_stats.active_tile_steps: every tile of an all-wet mesh is active at every step; on the
+    wet-dry dam break the dry end of the canal is not, and the count grows as the front advances."""
+    w = W.config1()
+    m = B.SweMesh.from_workload(w).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    m.run(50)
+    assert m.get_stats()["active_tile_steps"] == 50 * m.get_tile_info()["ntiles"]
+    w = W.config2(nx=600, ny=60)
+    m = B.SweMesh.from_workload(w, loop_mode=B.LOOP_PERSISTENT).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    nt = m.get_tile_info()["ntiles"]
+    m.run(100)
+    a1 = m.get_stats()["active_tile_steps"]
+    m.run(100)
+    a2 = m.get_stats()["active_tile_steps"] - a1
+    assert 0.4 * 100 * nt < a1 < a2 < 100 * nt
