@@ -103,7 +103,7 @@ int swe_params_default(swe_params *p);
  *   bc_tags     host [nt][3]  boundary tag per local edge, read only where the edge has no
  *                             neighbour; <= 0 or missing means SWE_BC_WALL
  *   params      host          NULL = defaults
- * Tables built (in the internal cell order): per-tile edge lists (end points, unit normal, length),
+ * Tables built (in the internal cell order): per-tile edge lists (end points, length-scaled normal),
  * halo lists, 1 / |Omega_i|, 1 / R_i, g m^2, cell bed.  nt < 2^29.  No CUDA call is made.
  */
 int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_t nt,
