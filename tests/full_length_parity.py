@@ -1,6 +1,6 @@
 """Full-size, full-length parity run (minutes of CPU time, so not part of the pytest suite):
 
-    python -m tests.full_length_parity config3 config4
+    python -m tests.full_length_parity config3 config4 sweep_50M
 
 Runs BASELINE.json's config at its full size for its full step count on the GPU (bench.py's
 launch configuration) and on the CPU oracle, and prints the largest deviations in the terms of
@@ -20,7 +20,10 @@ from paper_2010_14416_b200 import workloads as W
 def main(names):
     ok = True
     for name in names:
-        w = {"config1": W.config1, "config2": W.config2, "config3": W.config3, "config4": W.config4}[name]()
+        if name.startswith("sweep_"):            # config 5: sweep_0.1M ... sweep_50M
+            w = W.config5(name[len("sweep_"):])
+        else:
+            w = {"config1": W.config1, "config2": W.config2, "config3": W.config3, "config4": W.config4}[name]()
         t0 = time.time()
         m = B.SweMesh.from_workload(w).bind_device()
         m.set_state(w.h, w.hu, w.hv)
