@@ -7,10 +7,28 @@
 #include <cmath>
 #include <cstdio>
 #include <numeric>
+#include <thread>
 
 namespace swe {
 
 namespace {
+
+// Static partition of [0, n) over the host threads (at most 16); fn(begin, end, thread).  The
+// results never depend on the number of threads: every loop below writes disjoint outputs.
+template <class F> void parallel_for(int64_t n, F fn, int64_t grain = 65536)
+{
+    int nthr = (int)std::min<int64_t>(std::min<unsigned>(std::max(1u, std::thread::hardware_concurrency()), 16u),
+                                      std::max<int64_t>(1, n / grain));
+    if (nthr <= 1) { fn((int64_t)0, n, 0); return; }
+    std::vector<std::thread> pool;
+    const int64_t chunk = (n + nthr - 1) / nthr;
+    for (int t = 0; t < nthr; t++) {
+        const int64_t b = std::min<int64_t>(n, t * chunk), e = std::min<int64_t>(n, b + chunk);
+        pool.emplace_back([=, &fn] { fn(b, e, t); });
+    }
+    for (auto &th : pool) th.join();
+}
+constexpr int kMaxHostThreads = 16;
 
 // Hilbert index of (x, y) on a 2^order x 2^order grid (classic rotate-and-flip walk).
 inline uint32_t hilbert_d(uint32_t x, uint32_t y, int order)
@@ -39,12 +57,22 @@ void order_hilbert(HostTables &T)
     const int order = 16;
     const double ext = std::max(std::max(xmax - xmin, ymax - ymin), 1e-300);
     const double scale = (double)((1u << order) - 1) / ext; // square curve cells
-    std::vector<uint64_t> key((size_t)nt);
-    for (int64_t i = 0; i < nt; i++) {
-        uint32_t qx = (uint32_t)((T.cx[i] - xmin) * scale), qy = (uint32_t)((T.cy[i] - ymin) * scale);
-        key[(size_t)i] = ((uint64_t)hilbert_d(qx, qy, order) << 32) | (uint64_t)(uint32_t)i;
+    std::vector<uint64_t> key((size_t)nt), tmp((size_t)nt);
+    parallel_for(nt, [&](int64_t b, int64_t e, int) {
+        for (int64_t i = b; i < e; i++) {
+            uint32_t qx = (uint32_t)((T.cx[i] - xmin) * scale), qy = (uint32_t)((T.cy[i] - ymin) * scale);
+            key[(size_t)i] = ((uint64_t)hilbert_d(qx, qy, order) << 32) | (uint64_t)(uint32_t)i;
+        }
+    });
+    // stable LSD radix sort on the curve index (bits 32-63); the low word is the caller id in
+    // ascending order to begin with, so ties stay broken by caller id: deterministic
+    for (int shift = 32; shift < 64; shift += 8) {
+        size_t count[257] = {};
+        for (int64_t i = 0; i < nt; i++) count[((key[(size_t)i] >> shift) & 0xff) + 1]++;
+        for (int b = 0; b < 256; b++) count[b + 1] += count[b];
+        for (int64_t i = 0; i < nt; i++) tmp[count[(key[(size_t)i] >> shift) & 0xff]++] = key[(size_t)i];
+        key.swap(tmp);
     }
-    std::sort(key.begin(), key.end()); // ties broken by caller id: deterministic
     for (int64_t p = 0; p < nt; p++) T.perm[(size_t)p] = (int32_t)(key[(size_t)p] & 0xffffffffu);
 }
 
@@ -115,16 +143,18 @@ int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_
     // ---- orientation + geometry; vertices after the CCW fix kept for edge matching
     std::vector<int32_t> vtx(3 * (size_t)nt);
     std::vector<int8_t> tag(3 * (size_t)nt);
-    for (int64_t i = 0; i < nt; i++) {
+    // first offending triangle per thread: {index, status}; the smallest index is reported
+    int64_t bad_i[kMaxHostThreads]; int bad_rc[kMaxHostThreads];
+    for (int t = 0; t < kMaxHostThreads; t++) { bad_i[t] = INT64_MAX; bad_rc[t] = SWE_OK; }
+    parallel_for(nt, [&](int64_t begin, int64_t end, int thr) {
+    for (int64_t i = begin; i < end; i++) {
         int32_t v0 = tris[3 * i], v1 = tris[3 * i + 1], v2 = tris[3 * i + 2];
         int8_t t0 = bc_tags[3 * i], t1 = bc_tags[3 * i + 1], t2 = bc_tags[3 * i + 2];
         if (v0 < 0 || v0 >= nn || v1 < 0 || v1 >= nn || v2 < 0 || v2 >= nn) {
-            snprintf(msg, sizeof msg, "triangle %lld refers to a node outside [0, %lld)", (long long)i, (long long)nn);
-            err = msg; return SWE_ERR_BAD_INDEX;
+            bad_i[thr] = i; bad_rc[thr] = SWE_ERR_BAD_INDEX; return;
         }
         if (!(manning[i] >= 0.0) || !std::isfinite(manning[i])) {
-            snprintf(msg, sizeof msg, "cell %lld has a negative or non-finite Manning coefficient", (long long)i);
-            err = msg; return SWE_ERR_BAD_VALUE;
+            bad_i[thr] = i; bad_rc[thr] = SWE_ERR_BAD_VALUE; return;
         }
         double ax = nodes_xy[2 * (size_t)v0], ay = nodes_xy[2 * (size_t)v0 + 1];
         double bx = nodes_xy[2 * (size_t)v1], by = nodes_xy[2 * (size_t)v1 + 1];
@@ -134,10 +164,7 @@ int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_
             std::swap(v1, v2); std::swap(bx, cx); std::swap(by, cy); std::swap(t0, t2);
             twiceA = (bx - ax) * (cy - ay) - (cx - ax) * (by - ay);
         }
-        if (!(twiceA > 0.0)) {
-            snprintf(msg, sizeof msg, "triangle %lld has zero area", (long long)i);
-            err = msg; return SWE_ERR_DEGENERATE;
-        }
+        if (!(twiceA > 0.0)) { bad_i[thr] = i; bad_rc[thr] = SWE_ERR_DEGENERATE; return; }
         const double px[4] = { ax, bx, cx, ax }, py[4] = { ay, by, cy, ay };
         double perimeter = 0.0;
         for (int k = 0; k < 3; k++) {
@@ -156,6 +183,21 @@ int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_
         T.cx[(size_t)i] = (ax + bx + cx) / 3.0; T.cy[(size_t)i] = (ay + by + cy) / 3.0;
         vtx[3 * (size_t)i] = v0; vtx[3 * (size_t)i + 1] = v1; vtx[3 * (size_t)i + 2] = v2;
         tag[3 * (size_t)i] = t0; tag[3 * (size_t)i + 1] = t1; tag[3 * (size_t)i + 2] = t2;
+    }
+    });
+    {
+        int worst = 0;
+        for (int t = 1; t < kMaxHostThreads; t++) if (bad_i[t] < bad_i[worst]) worst = t;
+        if (bad_rc[worst] != SWE_OK) {
+            const long long i = (long long)bad_i[worst];
+            if (bad_rc[worst] == SWE_ERR_BAD_INDEX)
+                snprintf(msg, sizeof msg, "triangle %lld refers to a node outside [0, %lld)", i, (long long)nn);
+            else if (bad_rc[worst] == SWE_ERR_BAD_VALUE)
+                snprintf(msg, sizeof msg, "cell %lld has a negative or non-finite Manning coefficient", i);
+            else
+                snprintf(msg, sizeof msg, "triangle %lld has zero area", i);
+            err = msg; return bad_rc[worst];
+        }
     }
     // ---- edge matching: bucket the 3 nt half-edges by their smaller node id (counting sort),
     //      then pair equal larger ids inside each (tiny) bucket
@@ -176,7 +218,10 @@ int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_
         std::vector<int64_t> slot(ne);
         for (size_t e = 0; e < ne; e++) slot[(size_t)fill[(size_t)lo_of(e)]++] = (int64_t)e;
         std::fill(T.nbr.begin(), T.nbr.end(), INT32_MIN);
-        for (int64_t n = 0; n < nn; n++) {
+        int64_t bad_n[kMaxHostThreads], bad_hi[kMaxHostThreads];
+        for (int t = 0; t < kMaxHostThreads; t++) { bad_n[t] = INT64_MAX; bad_hi[t] = 0; }
+        parallel_for(nn, [&](int64_t nbegin, int64_t nend, int thr) {
+        for (int64_t n = nbegin; n < nend; n++) {
             for (int64_t a = start[(size_t)n]; a < start[(size_t)n + 1]; a++) {
                 const size_t ea = (size_t)slot[(size_t)a];
                 int matches = 0;
@@ -188,18 +233,23 @@ int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_
                         T.nbr[ea] = (int32_t)(eb / 3);
                     }
                 }
-                if (matches > 1) {
-                    snprintf(msg, sizeof msg, "edge (%d,%d) is shared by more than two triangles", (int)n, (int)hi_of(ea));
-                    err = msg; return SWE_ERR_NON_MANIFOLD;
-                }
+                if (matches > 1) { bad_n[thr] = n; bad_hi[thr] = hi_of(ea); return; }
                 if (matches == 0) {
                     int t = tag[ea];
                     if (t <= 0) t = SWE_BC_WALL; // untagged boundary edge
                     T.nbr[ea] = -t;
-                    T.inflow_length[t] += T.length[ea];
                 }
             }
         }
+        });
+        int worst = 0;
+        for (int t = 1; t < kMaxHostThreads; t++) if (bad_n[t] < bad_n[worst]) worst = t;
+        if (bad_n[worst] != INT64_MAX) {
+            snprintf(msg, sizeof msg, "edge (%d,%d) is shared by more than two triangles", (int)bad_n[worst], (int)bad_hi[worst]);
+            err = msg; return SWE_ERR_NON_MANIFOLD;
+        }
+        // total boundary length per tag, summed in (cell, local edge) order whatever the threads did
+        for (size_t e = 0; e < ne; e++) if (T.nbr[e] < 0) T.inflow_length[-T.nbr[e]] += T.length[e];
     }
     // ---- locality renumbering of the cells (edge order inside each cell is preserved, R-17)
     if (ordering == SWE_ORDER_HILBERT) order_hilbert(T);
@@ -223,10 +273,8 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
         std::vector<int32_t> hstart((size_t)X.ntiles + 1, 0), halo, ecount((size_t)X.ntiles, 0);
         X.nedges = 0;
         X.max_halo = 0;
-        std::vector<int32_t> halo_tile((size_t)nt, -1), halo_slot((size_t)nt, 0);
         X.cellc.assign((size_t)X.ntiles * 3 * TC, 1.0);
         X.edges.clear();
-        X.edges.reserve((size_t)nt * 7 / 4 + 1024);
         X.max_edges = 0;
         auto local_edge_towards = [&](int32_t c, int32_t other) {   // k with nbr(c,k) == other
             for (int k = 0; k < 3; k++) if (T.nbr[3 * (size_t)c + k] == other) return k;
@@ -239,59 +287,96 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
         for (size_t e = 0; e < 3 * (size_t)nt; e++)
             if (T.nbr[e] < 0) { bnum[e] = (int32_t)X.nbedges++; X.btag.push_back(-T.nbr[e]); }
         if (X.nbedges >= ((int64_t)1 << 24)) { err = "more than 2^24 boundary edges"; return SWE_ERR_INVALID_ARG; }
-        for (int64_t t = 0; t < X.ntiles; t++) {
-            const int64_t base = t * TC, nc = std::min<int64_t>(TC, nt - base);
-            const size_t first = X.edges.size(), hfirst = halo.size();
-            // position of internal cell pj in the tile's record array
-            auto pos = [&](int64_t pj) -> int64_t {
-                if (pj >= base && pj < base + TC) return pj - base;
-                if (halo_tile[(size_t)pj] != (int32_t)t) {
-                    halo_tile[(size_t)pj] = (int32_t)t;
-                    halo_slot[(size_t)pj] = (int32_t)(halo.size() - hfirst);
-                    halo.push_back((int32_t)pj);
-                }
-                return TC + halo_slot[(size_t)pj];
-            };
-            double *cc = X.cellc.data() + (size_t)t * 3 * TC;
-            for (int64_t q = 0; q < TC; q++) cc[2 * TC + q] = 0.0;
-            for (int64_t q = 0; q < nc; q++) {
-                const int64_t p = base + q;
-                const int32_t c = T.perm[(size_t)p];
-                for (int k = 0; k < 3; k++) {
-                    const int32_t j = T.nbr[3 * (size_t)c + k];
-                    const double *nk = &T.normal[6 * (size_t)c + 2 * k];
-                    if (j < 0) {                                   // boundary edge: a = this cell
-                        { const double L = T.length[3 * (size_t)c + k];
-                          X.edges.push_back({ enc(q, k), -((-j) + 128 * bnum[3 * (size_t)c + k]), L * nk[0], L * nk[1] }); }
-                        continue;
+        // The tiles are independent: every host thread builds the lists of a contiguous range of
+        // tiles into its own vectors, which are then laid end to end in tile order, so the tables do
+        // not depend on the number of threads.
+        struct Chunk { int64_t tb = 0, te = 0; std::vector<HostEdge> edges; std::vector<int32_t> halo; bool bad = false; };
+        std::vector<Chunk> chunks(kMaxHostThreads);
+        std::vector<int32_t> epad((size_t)X.ntiles, 0), hcount((size_t)X.ntiles, 0);
+        parallel_for(X.ntiles, [&](int64_t tb, int64_t te, int thr) {
+            Chunk &C = chunks[(size_t)thr];
+            C.tb = tb; C.te = te;
+            C.edges.reserve((size_t)(te - tb) * TC * 7 / 4 + 1024);
+            // off-tile cell -> halo slot of the current tile: open addressing, stamped by tile
+            const size_t hmask = 8191;                      // > 4 x (3 x 1024 cells) never needed: 3 TC <= 3072
+            std::vector<int64_t> hkey(hmask + 1, -1); std::vector<int32_t> hslot(hmask + 1, 0), hstamp(hmask + 1, -1);
+            for (int64_t t = tb; t < te; t++) {
+                const int64_t base = t * TC, nc = std::min<int64_t>(TC, nt - base);
+                const size_t first = C.edges.size(), hfirst = C.halo.size();
+                // position of internal cell pj in the tile's record array
+                auto pos = [&](int64_t pj) -> int64_t {
+                    if (pj >= base && pj < base + TC) return pj - base;
+                    size_t k = (size_t)((uint64_t)pj * 0x9E3779B97F4A7C15ull >> 40) & hmask;
+                    while (hstamp[k] == (int32_t)t && hkey[k] != pj) k = (k + 1) & hmask;
+                    if (hstamp[k] != (int32_t)t) {
+                        hstamp[k] = (int32_t)t; hkey[k] = pj;
+                        hslot[k] = (int32_t)(C.halo.size() - hfirst);
+                        C.halo.push_back((int32_t)pj);
                     }
-                    const int64_t pj = T.inv[(size_t)j];
-                    const bool in_tile = pj >= base && pj < base + nc;
-                    if (in_tile && pj < p) continue;               // emitted when pj was visited
-                    const int kj = local_edge_towards(j, c);
-                    if (kj < 0) { err = "inconsistent neighbour table"; return SWE_ERR_NON_MANIFOLD; }
-                    if (c < j)                                     // a = smaller caller id (R-17)
-                        { const double L = T.length[3 * (size_t)c + k];
-                          X.edges.push_back({ enc(q, k), enc(pos(pj), kj), L * nk[0], L * nk[1] }); }
-                    else
-                        { const double L = T.length[3 * (size_t)j + kj];
-                          X.edges.push_back({ enc(pos(pj), kj), enc(q, k), L * T.normal[6 * (size_t)j + 2 * kj],
-                                              L * T.normal[6 * (size_t)j + 2 * kj + 1] }); }
+                    return TC + hslot[k];
+                };
+                double *cc = X.cellc.data() + (size_t)t * 3 * TC;
+                for (int64_t q = 0; q < TC; q++) cc[2 * TC + q] = 0.0;
+                for (int64_t q = 0; q < nc; q++) {
+                    const int64_t p = base + q;
+                    const int32_t c = T.perm[(size_t)p];
+                    for (int k = 0; k < 3; k++) {
+                        const int32_t j = T.nbr[3 * (size_t)c + k];
+                        const double *nk = &T.normal[6 * (size_t)c + 2 * k];
+                        if (j < 0) {                                   // boundary edge: a = this cell
+                            const double L = T.length[3 * (size_t)c + k];
+                            C.edges.push_back({ enc(q, k), -((-j) + 128 * bnum[3 * (size_t)c + k]), L * nk[0], L * nk[1] });
+                            continue;
+                        }
+                        const int64_t pj = T.inv[(size_t)j];
+                        const bool in_tile = pj >= base && pj < base + nc;
+                        if (in_tile && pj < p) continue;               // emitted when pj was visited
+                        const int kj = local_edge_towards(j, c);
+                        if (kj < 0) { C.bad = true; return; }
+                        if (c < j) {                                   // a = smaller caller id (R-17)
+                            const double L = T.length[3 * (size_t)c + k];
+                            C.edges.push_back({ enc(q, k), enc(pos(pj), kj), L * nk[0], L * nk[1] });
+                        } else {
+                            const double L = T.length[3 * (size_t)j + kj];
+                            C.edges.push_back({ enc(pos(pj), kj), enc(q, k), L * T.normal[6 * (size_t)j + 2 * kj],
+                                                L * T.normal[6 * (size_t)j + 2 * kj + 1] });
+                        }
+                    }
+                    cc[q] = 1.0 / T.area[(size_t)c];
+                    cc[TC + q] = 1.0 / T.inradius[(size_t)c];
+                    cc[2 * TC + q] = g * T.manning[(size_t)c] * T.manning[(size_t)c];
                 }
-                cc[q] = 1.0 / T.area[(size_t)c];
-                cc[TC + q] = 1.0 / T.inradius[(size_t)c];
-                cc[2 * TC + q] = g * T.manning[(size_t)c] * T.manning[(size_t)c];
+                const size_t cnt = C.edges.size() - first;
+                ecount[(size_t)t] = (int32_t)cnt;
+                if (cnt & 1) C.edges.push_back({ 0, 0, 0.0, 0.0 });       // pad to 16-byte granules
+                epad[(size_t)t] = (int32_t)(C.edges.size() - first);
+                hcount[(size_t)t] = (int32_t)(C.halo.size() - hfirst);
             }
-            const size_t cnt = X.edges.size() - first;
-            ecount[(size_t)t] = (int32_t)cnt;
-            X.nedges += (int64_t)cnt;
-            if (cnt & 1) X.edges.push_back({ 0, 0, 0.0, 0.0 });       // pad to 16-byte granules
-            if (X.edges.size() > (size_t)INT32_MAX) { err = "too many edges"; return SWE_ERR_INVALID_ARG; }
-            X.max_edges = std::max<int32_t>(X.max_edges, (int32_t)(X.edges.size() - first));
-            X.estart[(size_t)t + 1] = (int32_t)X.edges.size();
-            if (halo.size() > (size_t)INT32_MAX) { err = "too many halo cells"; return SWE_ERR_INVALID_ARG; }
-            X.max_halo = std::max<int32_t>(X.max_halo, (int32_t)(halo.size() - hfirst));
-            hstart[(size_t)t + 1] = (int32_t)halo.size();
+        }, 256);
+        for (const Chunk &C : chunks) if (C.bad) { err = "inconsistent neighbour table"; return SWE_ERR_NON_MANIFOLD; }
+        {
+            int64_t etot = 0, htot = 0;
+            for (int64_t t = 0; t < X.ntiles; t++) {
+                X.estart[(size_t)t] = (int32_t)etot; hstart[(size_t)t] = (int32_t)htot;
+                etot += epad[(size_t)t]; htot += hcount[(size_t)t];
+                X.nedges += ecount[(size_t)t];
+                X.max_edges = std::max(X.max_edges, epad[(size_t)t]);
+                X.max_halo = std::max(X.max_halo, hcount[(size_t)t]);
+            }
+            if (etot > (int64_t)INT32_MAX) { err = "too many edges"; return SWE_ERR_INVALID_ARG; }
+            if (htot > (int64_t)INT32_MAX) { err = "too many halo cells"; return SWE_ERR_INVALID_ARG; }
+            X.estart[(size_t)X.ntiles] = (int32_t)etot; hstart[(size_t)X.ntiles] = (int32_t)htot;
+            X.edges.resize((size_t)etot); halo.resize((size_t)htot);
+            std::vector<std::thread> pool;
+            for (Chunk &C : chunks) {
+                if (C.te <= C.tb) continue;
+                pool.emplace_back([&X, &halo, &hstart, &C] {
+                    std::copy(C.edges.begin(), C.edges.end(), X.edges.begin() + X.estart[(size_t)C.tb]);
+                    std::copy(C.halo.begin(), C.halo.end(), halo.begin() + hstart[(size_t)C.tb]);
+                    std::vector<HostEdge>().swap(C.edges);
+                });
+            }
+            for (auto &th : pool) th.join();
         }
         // fixed-stride info blocks (16-byte granules for the bulk copy)
         X.max_halo = (X.max_halo + 3) / 4 * 4;
