@@ -7,6 +7,8 @@
 #include <cmath>
 #include <cstdio>
 #include <numeric>
+#include <atomic>
+#include <new>
 #include <thread>
 
 namespace swe {
@@ -21,12 +23,14 @@ template <class F> void parallel_for(int64_t n, F fn, int64_t grain = 65536)
                                       std::max<int64_t>(1, n / grain));
     if (nthr <= 1) { fn((int64_t)0, n, 0); return; }
     std::vector<std::thread> pool;
+    std::atomic<bool> failed(false);
     const int64_t chunk = (n + nthr - 1) / nthr;
     for (int t = 0; t < nthr; t++) {
         const int64_t b = std::min<int64_t>(n, t * chunk), e = std::min<int64_t>(n, b + chunk);
-        pool.emplace_back([=, &fn] { fn(b, e, t); });
+        pool.emplace_back([=, &fn, &failed] { try { fn(b, e, t); } catch (...) { failed = true; } });
     }
     for (auto &th : pool) th.join();
+    if (failed) throw std::bad_alloc();      // the only thing these loops can throw
 }
 constexpr int kMaxHostThreads = 16;
 
