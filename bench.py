@@ -127,6 +127,7 @@ def time_oracle(w, steps: int, warmup: int, threads=None):
     """The oracle as it stands on the host cores: returns (cell-updates/s, threads used)."""
     from oracle.swe_oracle import OracleSolver
     o = OracleSolver.from_workload(w)
+    one_thread = None
     if threads is None:   # pick the thread count that is actually fastest on this box
         best = (0.0, 1)
         for n in sorted({1, 2, 4, 8, 16, 32, os.cpu_count() or 1}):
@@ -138,6 +139,8 @@ def time_oracle(w, steps: int, warmup: int, threads=None):
             t0 = time.perf_counter()
             o.run(3)
             r = 3 * w.ncells / (time.perf_counter() - t0)
+            if n == 1:
+                one_thread = r
             if r > best[0]:
                 best = (r, n)
         threads = best[1]
@@ -148,6 +151,7 @@ def time_oracle(w, steps: int, warmup: int, threads=None):
     t0 = time.perf_counter()
     done = o.run(steps)
     dt = time.perf_counter() - t0
+    time_oracle.one_thread = one_thread        # 3-step probe with a single thread
     return done * w.ncells / dt, threads, dt
 
 
@@ -296,7 +300,8 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                      "kernel": f"swe_step_kernel<{tiles['tile_cells']}>", "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
                      "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
         "cpu_baseline": {"value": cpu_value, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
-                         "sample": what},
+                         "sample": what, "value_1_thread": getattr(time_oracle, "one_thread", None),
+                         "host_cores": os.cpu_count()},
         "e2e": {"value": total_updates / (e2e_ms * 1e-3), "unit": UNIT,
                 "h2d_bytes_per_step": 24.0 * n / args.steps, "d2h_bytes_per_step": 24.0 * n / args.steps,
                 "job": "swe_set_state(pinned host) + swe_run(K) + swe_get_state(pinned host); "
