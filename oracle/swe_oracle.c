@@ -31,8 +31,11 @@
  *   boundary volumes   : inflow tag = -Q t exactly, walls 0, tags add up to the total, volume
  *                        change = -sum; run_until: ends on t_end, equals run() before the last step
  *   dt                 : closed form CFL * R_min / (sqrt(g h) + |V|) on a uniform state
- *   unpinned conventions: R-1 cell bed = mean of node beds, R-2 g = 9.81,
- *                        R-6 clamp in eq. (22).
+ *   inflow flux        : uniform channel flow fed with Q = h u stays steady (momentum term
+ *                        Q^2/h + g h^2/2); dry inflow cell hand value
+ *   eq.(22) clamp R-6  : dry-bed-generating rarefactions: S_L = u_L - a_L, S_R = u_R + a_R exactly
+ *   eq.(24) R-16       : continuity of G_3 with eq.(17) as S_L -> 0-, S_R -> 0+
+ *   unpinned conventions: R-1 cell bed = mean of node beds, R-2 g = 9.81.
  */
 #include <math.h>
 #include <stdint.h>
@@ -452,10 +455,13 @@ int64_t oracle_run_until(oracle_mesh *m, double t_end, int64_t max_steps)
     int64_t done = 0;
     if (!m->dt_valid) oracle_compute_dt(m);
     while (done < max_steps && m->t < t_end) {
-        if (!(m->dt > 0.0)) break;
+        if (!(m->dt > 0.0) || !isfinite(m->dt)) break;
         double dt = m->dt;
-        if (t_end - m->t < dt) dt = t_end - m->t;
+        const int last = t_end - m->t <= dt;
+        if (last) dt = t_end - m->t;
+        if (!(m->t + dt > m->t)) break; /* a collapsed dt (blow-up) makes no progress: stop, do not spin */
         step(m, dt);
+        if (last) m->t = t_end;         /* R-24: the clipped step ends ON t_end (t + (t_end - t) may round off it) */
         oracle_compute_dt(m);
         done++;
     }

@@ -129,6 +129,51 @@ def test_pk_continuity():
     assert a["SR"] == pytest.approx(b["SR"], abs=1e-5)
 
 
+def test_eq22_clamp_dry_bed_generating_rarefactions():
+    """R-6 (eq.22): for strongly diverging states, u_R - u_L >= 2 (a_L + a_R), the exact
+    Riemann solution opens a dry bed between two rarefactions whose heads travel at exactly
+    u_L - a_L and u_R + a_R (Toro 2001, dry-bed generation), i.e. p_L = p_R = 1 in eq.(19).  The
+    bracket of eq.(22) is negative there; squaring it unclamped gives h* = 1.94 > h_k here and a
+    spurious "shock" factor p_k = 1.69, so the clamp at 0 is what reproduces the exact speeds."""
+    h, uL, uR = 1.0, -15.0, 15.0
+    a = math.sqrt(G * h)
+    assert uR - uL > 8.0 * a                 # bracket^2 / g > h: the unclamped reading differs
+    Gf, d = hllc(h, uL, 0.0, h, uR, 0.0)
+    assert d["branch"] == 3 and d["hs"] == 0.0
+    assert d["pL"] == 1.0 and d["pR"] == 1.0
+    assert d["SL"] == uL - a and d["SR"] == uR + a
+    # the same with unequal depths and a tangential velocity; the mass flux is the HLL average (18)
+    hL, hR = 0.7, 1.6
+    aL, aR = math.sqrt(G * hL), math.sqrt(G * hR)
+    Gf, d = hllc(hL, -22.0, 0.3, hR, 21.0, -0.2)
+    assert d["branch"] == 3 and d["hs"] == 0.0
+    assert d["SL"] == -22.0 - aL and d["SR"] == 21.0 + aR
+    SL, SR = d["SL"], d["SR"]
+    want = (SR * hL * -22.0 - SL * hR * 21.0 + SL * SR * (hR - hL)) / (SR - SL)
+    assert Gf[0] == pytest.approx(want, rel=1e-14)
+
+
+def test_eq24_continuous_with_eq17_across_SL_zero():
+    """R-16 (eq.24): the flux is a continuous function of the states, so as
+    S_L -> 0^- the star-region flux must tend to eq.(17)'s G(U_L) = (h u, ., h u v_L): the tangential
+    velocity is v_L for S* >= 0.  The inequality as printed (v_L for S* <= 0) would give h u v_R
+    here.  Mirror case: S_R -> 0^+ must tend to G(U_R)."""
+    h, vL, vR = 1.0, 0.7, -0.4
+    a = math.sqrt(G * h)
+    for eps in (1e-3, 1e-6, 1e-9):
+        u = a * (1.0 - eps)                   # equal depths and normal velocities: S_L = u - a = -eps a
+        Gf, d = hllc(h, u, vL, h, u, vR)
+        assert -2.0 * eps * a < d["SL"] < 0.0 and d["Sstar"] > 0.0
+        assert Gf[0] == pytest.approx(h * u, rel=1e-12)
+        assert Gf[2] == pytest.approx(h * u * vL, rel=1e-12)      # printed inequality: h u vR = -1.25
+        Gf, d = hllc(h, -u, vL, h, -u, vR)
+        assert 0.0 < d["SR"] < 2.0 * eps * a and d["Sstar"] < 0.0
+        assert Gf[2] == pytest.approx(-h * u * vR, rel=1e-12)
+    # and just on the other side of the switch, eq.(17) itself
+    Gf, d = hllc(h, a * (1.0 + 1e-9), vL, h, a * (1.0 + 1e-9), vR)
+    assert d["SL"] > 0.0 and Gf[2] == pytest.approx(h * a * vL, rel=1e-8)
+
+
 def test_stoker_golden_digits():
     rows = {}
     with open(os.path.join(HERE, "golden", "stoker_ritter.txt")) as f:
