@@ -263,6 +263,31 @@ int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_
     return SWE_OK;
 }
 
+void pack_device_edges(const TileTables &X, std::vector<double> &out)
+{
+    out.assign(3 * X.edges.size(), 0.0);
+    const int32_t TC = X.tile_cells;
+    const int32_t mask = (1 << kHostIdBits) - 1;
+    auto word = [TC, mask](int32_t v) -> uint32_t {
+        if (v < 0) return (uint32_t)v;                         // boundary: -(tag + 128 * boundary edge number)
+        const uint32_t pos = (uint32_t)(v & mask), k = (uint32_t)v >> kHostIdBits;
+        const uint32_t slot = pos < (uint32_t)TC ? k * (uint32_t)(TC + 1) + pos : kDevNoSlot;
+        return pos | (k << kDevKShift) | (slot << kDevSlotShift);
+    };
+    parallel_for(X.ntiles, [&](int64_t tb, int64_t te, int) {
+        for (int64_t t = tb; t < te; t++) {
+            const size_t e0 = (size_t)X.estart[(size_t)t], nep = (size_t)X.estart[(size_t)t + 1] - e0;
+            uint32_t *ab = reinterpret_cast<uint32_t *>(out.data() + 3 * e0);
+            double *lxy = out.data() + 3 * e0 + nep;
+            for (size_t e = 0; e < nep; e++) {
+                const HostEdge &E = X.edges[e0 + e];
+                ab[2 * e] = word(E.a); ab[2 * e + 1] = word(E.b);
+                lxy[2 * e] = E.lx; lxy[2 * e + 1] = E.ly;
+            }
+        }
+    }, 256);
+}
+
 // ---- tile tables: each tile's unique edge list and its cells' constants -------------------------
 int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, std::string &err)
 {

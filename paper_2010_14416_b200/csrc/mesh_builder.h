@@ -54,6 +54,15 @@ struct TileTables {
     std::vector<double> cellc;         // [ntiles][3][tile_cells]: 1/|Omega|, 1/R, g m^2 (padded with 1, 1, 0)
 };
 
+// The edge lists in the layout the step kernel reads (swe_kernels.cuh): per tile, nep = its padded
+// edge count, first nep (a, b) word pairs, then nep (lx, ly) pairs; 3 doubles per edge in all, so
+// estart still indexes it.  End point word: bits 0-12 position, bits 13-14 local edge k, bits 16-30
+// flux slot k * (tile_cells + 1) + position for a cell of the tile, kDevNoSlot for a halo cell;
+// boundary words (negative) are kept.
+constexpr uint32_t kDevPosMask = 0x1FFFu, kDevNoSlot = 0x7FFFu;
+constexpr int kDevKShift = 13, kDevSlotShift = 16;
+void pack_device_edges(const TileTables &X, std::vector<double> &out);
+
 // Returns SWE_OK or a negative swe_status with a message in err.
 int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, std::string &err);
 

@@ -25,7 +25,7 @@ constexpr int kMaxBlock = 256;
 #define SWE_MIN_BLOCKS 3
 #endif
 constexpr int kMaxPart = 8192;       // upper bound on the grid of the step kernel
-extern __shared__ __align__(32) unsigned char dyn_smem[];
+extern __shared__ __align__(128) unsigned char dyn_smem[];
 
 // nsteps time steps.  Every block first reduces the per-block maxima of the previous step into
 // dt (redundantly: a few KB from L2), so no separate finaliser launch and no atomics sit between
@@ -40,10 +40,9 @@ __global__ void __launch_bounds__(TC, (SWE_MIN_BLOCKS * kMaxBlock) / TC)
 swe_step_kernel(const Params P, int cur, const long long nsteps)
 {
     __shared__ double s_red[32];
-    const TilePipe<TC> pp = make_pipe<TC>(P, dyn_smem);
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kNumBars; s++) mbar_init(pp.bar + s, 1);
-        pp.ecnt()[0] = 0; pp.ecnt()[1] = 0; *pp.nact() = 0;
+        uint64_t *bar = reinterpret_cast<uint64_t *>(dyn_smem + SmemLayout<TC>::bar);
+        for (int s = 0; s < kNumBars; s++) mbar_init(bar + s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -52,20 +51,20 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
         const double dt_cfl = reduce_dt(P, P.pmax(cur), s_red);
         // swe_run_until: the step that would pass t_end ends on it; after that, zero steps
         const double t_now = __ldcg(&P.ctrl->t[cur]);
-        const double dt = fmax(fmin(dt_cfl, __ldcg(&P.ctrl->t_end) - t_now), 0.0);
-        unsigned nclamp = 0;
-        double rate = step_tiles<TC>(P, pp, P.U(cur), P.U(cur ^ 1), dt, nclamp, it);
+        const double left = __ldcg(&P.ctrl->t_end) - t_now;
+        const bool clipped = dt_cfl >= left;
+        const double dt = fmax(clipped ? left : dt_cfl, 0.0);
+        unsigned nclamp = 0, nactive = 0;
+        double rate = step_tiles<TC>(P, dyn_smem, P.U(cur), P.U(cur ^ 1), dt, nclamp, nactive, it);
         rate = block_max(rate, s_red);
         if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
-        if (threadIdx.x == TC - 32 && *pp.nact()) {                               // likewise
-            atomicAdd(&P.ctrl->n_active, (unsigned long long)*pp.nact());
-            *pp.nact() = 0;
-        }
+        if (nactive) atomicAdd(&P.ctrl->n_active, (unsigned long long)nactive);  // likewise (producer thread)
         if (threadIdx.x == 0) {
             P.pmax(cur ^ 1)[blockIdx.x] = rate;
             if (blockIdx.x == 0) {
                 Ctrl *c = P.ctrl;
-                c->t[cur ^ 1] = t_now + dt;
+                // R-24: the clipped step ends ON t_end (t + (t_end - t) may round off it)
+                c->t[cur ^ 1] = clipped ? fmax(__ldcg(&P.ctrl->t_end), t_now) : t_now + dt;
                 if (dt > 0.0) { c->dt_last = dt; c->steps += 1; }
                 if (!(dt_cfl > 0.0)) c->all_dry = 1;
             }
@@ -188,7 +187,8 @@ static thread_local std::string g_create_err;
 static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 namespace {
-static_assert(sizeof(HostEdge) == sizeof(EdgeRec) && kHostIdBits == kIdBits, "table records");
+static_assert(sizeof(HostEdge) == 24 && kDevPosMask == kPosMask && kDevKShift == kKShift && kDevSlotShift == kSlotShift &&
+              kDevNoSlot == kNoSlot, "edge list encoding (mesh_builder.h / swe_kernels.cuh)");
 struct Layout {
     size_t U0, U1, cellc, edges, tinfo, bvol, hint, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
 };
@@ -197,10 +197,10 @@ Layout make_layout(const HostTables &T, const TileTables &X)
     Layout L; size_t o = 0; const size_t n = (size_t)T.nt;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
     L.U0 = take(n * sizeof(Rec)); L.U1 = take(n * sizeof(Rec));
-    L.cellc = take(X.cellc.size() * sizeof(double)); L.edges = take(X.edges.size() * sizeof(EdgeRec));
+    L.cellc = take(X.cellc.size() * sizeof(double)); L.edges = take(X.edges.size() * sizeof(HostEdge));
     L.tinfo = take(X.tinfo.size() * sizeof(int32_t));
     L.bvol = take(((size_t)X.nbedges + 1) * sizeof(double));
-    L.hint = take(((size_t)X.ntiles + 1) * sizeof(int4));
+    L.hint = take(((size_t)X.ntiles + 1) * sizeof(int32_t));
     L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
     L.stage = take(3 * n * sizeof(double));
     L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
@@ -391,10 +391,10 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
 
     Params &P = m->P;
     P.U0 = (Rec *)(m->ws + L.U0); P.U1 = (Rec *)(m->ws + L.U1);
-    P.cellc = (const double *)(m->ws + L.cellc); P.edges = (const EdgeRec *)(m->ws + L.edges);
+    P.cellc = (const double *)(m->ws + L.cellc); P.edges = (const double *)(m->ws + L.edges);
     P.tinfo = (const int32_t *)(m->ws + L.tinfo);
     P.bvol = (double *)(m->ws + L.bvol);
-    P.hint = (int4 *)(m->ws + L.hint);
+    P.hint = (int32_t *)(m->ws + L.hint);
     m->d_zcell = (double *)(m->ws + L.zcell); m->d_inv = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
@@ -411,7 +411,9 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     try {
         cudaStream_t s = m->stream;
         CK(cudaMemcpyAsync(m->ws + L.cellc, X.cellc.data(), X.cellc.size() * sizeof(double), cudaMemcpyHostToDevice, s));
-        CK(cudaMemcpyAsync(m->ws + L.edges, X.edges.data(), X.edges.size() * sizeof(EdgeRec), cudaMemcpyHostToDevice, s));
+        std::vector<double> dev_edges;          // the edge lists as the kernel reads them (freed after the upload)
+        pack_device_edges(X, dev_edges);
+        CK(cudaMemcpyAsync(m->ws + L.edges, dev_edges.data(), dev_edges.size() * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.tinfo, X.tinfo.data(), X.tinfo.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_zcell, T.cell_z.data(), n * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_inv, T.inv.data(), n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
@@ -450,7 +452,7 @@ static int set_state_common(swe_mesh *m, const double *h, const double *hu, cons
     m->cur = 0;
     m->have_state = false; m->have_rates = false;
     Ctrl c{}; c.t[0] = t0; c.t[1] = t0; c.t_end = INFINITY; c.bad_cell = INT32_MAX;
-    CK(cudaMemsetAsync(m->P.hint, 1, (size_t)m->X.ntiles * sizeof(int4), m->stream));   // nothing known yet: every tile active (.x != 0)
+    CK(cudaMemsetAsync(m->P.hint, 1, (size_t)m->X.ntiles * sizeof(int32_t), m->stream));   // nothing known yet: every tile active (!= 0)
     if (m->X.nbedges > 0) CK(cudaMemsetAsync(m->P.bvol, 0, (size_t)m->X.nbedges * sizeof(double), m->stream));
     CK(cudaMemcpyAsync(m->P.ctrl, &c, sizeof(Ctrl), cudaMemcpyHostToDevice, m->stream));
     swe_pack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_inv, h, hu, hv, m->d_zcell);
