@@ -9,6 +9,12 @@ config and one of the ">= 4M-cell meshes" the north_star's roofline target is qu
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
 
+The line also carries a "wet" record: BASELINE.json configs[2] (lake at rest, 4,000,000 cells, every
+cell wet) timed the same way in the same process -- the regime in which every cell does the method's
+work and the kernel is furthest from the HBM roof.  roofline.frac charges 156 algorithmic bytes to the
+cells of active tiles and 64 bytes to the cells of all-dry tiles (counted on the device during the
+timed steps), so it cannot exceed ~1; the fixed-156 figure is kept as frac_fixed_156.
+
 N > 1 (torchrun): the path does not shard ("replicas only"): every rank runs the same
 workload independently, value = all ranks' cell-updates / max-over-ranks device time.
 """
@@ -67,20 +73,6 @@ def load_peaks():
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
-
-
-def load_traffic(workload: str):
-    """dram bytes per launch of the step kernel from the committed ncu --set full capture
-    (profiles/traffic.csv: workload,dram_bytes_per_launch; profiles/r01_v8_README.md says how)."""
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
-            for line in f.read().splitlines()[1:]:
-                name, val = line.split(",")
-                if name == workload:
-                    return int(val)
-    except Exception:
-        pass
-    return None
 
 
 class ClockSampler:
@@ -156,15 +148,16 @@ def time_oracle(w, steps: int, warmup: int, threads=None):
 
 
 def run_reference(args, rank: int, world: int):
-    """--impl reference: the oracle, as it stands, on the box's host cores (rank 0 only)."""
+    """--impl reference: the oracle, as it stands, on the box's host cores (rank 0 only), with the
+    warm-up and step counts it was asked for (a step of the bounded sample takes milliseconds)."""
     if rank != 0:
         return
     sample, what = make_sample(args.workload)
-    steps = max(1, min(args.steps, 20))
-    value, threads, secs = time_oracle(sample, steps, min(args.warmup, 3))
+    steps = max(1, args.steps)
+    value, threads, secs = time_oracle(sample, steps, args.warmup)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": steps, "warmup": min(args.warmup, 3), "ms_per_step": 1e3 * secs / steps,
+        "steps": steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": {"workload": args.workload, "sample": what},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": what},
@@ -189,6 +182,73 @@ def job_throughput(cells_per_rank: int, steps: int, world: int, ms_max: float) -
     return float(cells_per_rank) * steps * world / (ms_max * 1e-3)
 
 
+STATE_BYTES_DRY = 64.0        # an all-dry tile's update is the identity: its 32-byte records in and out
+
+
+def roofline_record(n, kernel_ms, active_share, list_share, step_bytes, tiles, peak, peak_src):
+    """HBM roofline of one launch of the step kernel (= one time step of the whole mesh).
+
+    frac cannot exceed ~1 for a correct kernel: it charges the SURVEY's 156 algorithmic bytes only
+    to the cells of tiles that did the method's work in the timed steps and 64 bytes (record in and
+    out) to the cells of all-dry tiles, whose update is the identity (counted on the device).
+    traffic = the bytes this launch requested from memory according to the library's own table
+    sizes and the same counters (swe_get_step_bytes), not a stored constant."""
+    sec = kernel_ms * 1e-3
+    algo = (ALGO_BYTES_PER_CELL * active_share + STATE_BYTES_DRY * (1.0 - active_share)) * n
+    fixed = ALGO_BYTES_PER_CELL * n
+    return {"bound": "hbm", "achieved": algo / sec / 1e9, "peak": peak, "unit": "GB/s",
+            "frac": algo / sec / 1e9 / peak, "traffic": step_bytes,
+            "traffic_kind": "bytes requested per launch, from the library's table sizes and this run's "
+                            "device counters (swe_get_step_bytes); ncu dram__bytes cross-check in profiles/",
+            "achieved_traffic": step_bytes / sec / 1e9, "frac_traffic": step_bytes / sec / 1e9 / peak,
+            "algorithmic_bytes_per_launch": algo, "algorithmic_bytes_per_cell_active_tile": ALGO_BYTES_PER_CELL,
+            "algorithmic_bytes_per_cell_dry_tile": STATE_BYTES_DRY,
+            "active_tile_share": active_share, "edge_list_share": list_share,
+            "achieved_fixed_156": fixed / sec / 1e9, "frac_fixed_156": fixed / sec / 1e9 / peak,
+            "frac_of_nominal_8TBs": algo / sec / 1e9 / 8000.0,
+            "kernel": f"swe_step_kernel<{tiles['tile_cells']}>", "peak_source": peak_src}
+
+
+def measure_device(B, w, args, dev, order, loop, barrier, world, sampler=None):
+    """W warm-up steps, then exactly K timed steps in one swe_run, CUDA events on the mesh's stream."""
+    import torch
+    n = w.ncells
+    t_build = time.perf_counter()
+    m = B.SweMesh.from_workload(w, ordering=order, loop_mode=loop, block_size=args.block).bind_device(dev)
+    t_build = time.perf_counter() - t_build
+    m.set_state(w.h, w.hu, w.hv)
+    m.run(args.warmup)
+    for _ in range(2 if args.steps % 2 else 1):   # untimed: instantiates every CUDA graph the timed
+        m.run(args.steps)                          # call will replay (graphs are keyed by buffer parity)
+    m.sync()
+    launches0 = m.get_launch_info()["kernel_launches"]
+    st0 = m.get_stats()
+    if sampler is not None:
+        sampler.start()
+        time.sleep(0.25)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.time()
+    ev0.record(m.stream)
+    m.run(args.steps)
+    ev1.record(m.stream)
+    barrier()
+    t1 = time.time()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop(t0, t1) if sampler is not None else None
+    info = m.get_launch_info()
+    tiles = m.get_tile_info()
+    launches = info["kernel_launches"] - launches0 - 1          # minus the get_stats reduction above
+    st = m.get_stats()
+    tile_steps = float(tiles["ntiles"] * args.steps)
+    # share of (tile, step) pairs that were not all dry / whose edge list was read
+    active_share = (st["active_tile_steps"] - st0["active_tile_steps"]) / tile_steps
+    list_share = (st["edge_list_fetches"] - st0["edge_list_fetches"]) / tile_steps
+    step_bytes = m.get_step_bytes(active_share * tiles["ntiles"], list_share * tiles["ntiles"])
+    return dict(mesh=m, ms=ms, clocks=clocks, info=info, tiles=tiles, launches=launches, stats=st,
+                active_share=active_share, list_share=list_share, step_bytes=step_bytes, t_build=t_build)
+
+
 def run_gpu(args, rank: int, world: int, local_rank: int):
     import torch
     import torch.distributed as dist
@@ -201,55 +261,26 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     dev = f"cuda:{local_rank}"
 
-    w = make_workload(args.workload)
-    n = w.ncells
-    order = {"hilbert": B.ORDER_HILBERT, "rcm": B.ORDER_RCM, "identity": B.ORDER_IDENTITY}[args.ordering]
-    loop = {"auto": B.LOOP_AUTO, "graph": B.LOOP_GRAPH, "persistent": B.LOOP_PERSISTENT,
-            "launch": B.LOOP_LAUNCH}[args.loop]
-    t_build = time.perf_counter()
-    m = B.SweMesh.from_workload(w, ordering=order, loop_mode=loop, block_size=args.block).bind_device(dev)
-    t_build = time.perf_counter() - t_build
-    # pinned host buffers for the end-to-end leg
-    pin = [torch.empty(n, dtype=torch.float64).pin_memory() for _ in range(6)]
-    hin = [p.numpy() for p in pin[:3]]
-    hout = [p.numpy() for p in pin[3:]]
-    for dst, src in zip(hin, (w.h, w.hu, w.hv)):
-        dst[:] = src
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident leg: W warm-up steps, then exactly K timed steps in one swe_run ----
-    m.set_state(*hin)
-    m.run(args.warmup)
-    for _ in range(2 if args.steps % 2 else 1):   # untimed: instantiates every CUDA graph the timed
-        m.run(args.steps)                          # call will replay (graphs are keyed by buffer parity)
-    m.sync()
-    launches0 = m.get_launch_info()["kernel_launches"]
-    active0 = m.get_stats()["active_tile_steps"]
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    time.sleep(0.25)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    t0 = time.time()
-    ev0.record(m.stream)
-    m.run(args.steps)
-    ev1.record(m.stream)
-    barrier()
-    t1 = time.time()
-    ms = ev0.elapsed_time(ev1)
-    clocks = sampler.stop(t0, t1)
-    info = m.get_launch_info()
-    tiles = m.get_tile_info()
-    launches = info["kernel_launches"] - launches0
-    stats = m.get_stats()
-    # share of (tile, step) pairs that were not all dry: all-dry tiles copy their records (64 B/cell)
-    active_share = (stats["active_tile_steps"] - active0) / float(tiles["ntiles"] * args.steps)
+    w = make_workload(args.workload)
+    n = w.ncells
+    order = {"hilbert": B.ORDER_HILBERT, "rcm": B.ORDER_RCM, "identity": B.ORDER_IDENTITY}[args.ordering]
+    loop = {"auto": B.LOOP_AUTO, "graph": B.LOOP_GRAPH, "persistent": B.LOOP_PERSISTENT,
+            "launch": B.LOOP_LAUNCH}[args.loop]
+    # ---- device-resident leg of the headline workload -------------------------------------
+    r = measure_device(B, w, args, dev, order, loop, barrier, world, ClockSampler(local_rank))
+    m, ms, info, tiles, stats = r["mesh"], r["ms"], r["info"], r["tiles"], r["stats"]
 
     # ---- end-to-end leg through the C ABI with host buffers: set_state + run(K) + get_state ----
+    pin = [torch.empty(n, dtype=torch.float64).pin_memory() for _ in range(6)]
+    hin = [p.numpy() for p in pin[:3]]
+    hout = [p.numpy() for p in pin[3:]]
+    for dst, src in zip(hin, (w.h, w.hu, w.hv)):
+        dst[:] = src
     barrier()
     e0 = time.perf_counter()
     m.set_state(*hin)
@@ -257,8 +288,22 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     m.get_state_into(*hout)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - e0
+    m.destroy()
+    del pin, hin, hout
 
-    ms, e2e_ms = max_over_ranks([ms, e2e_s * 1e3], world, dev)
+    # ---- all-wet leg: BASELINE.json configs[2] (lake at rest, 4M cells, every cell does the
+    # method's work) timed the same way in the same process, so that the record carries the
+    # regime in which the kernel is furthest from the HBM roof ------------------------------
+    wet = None
+    if args.wet and args.workload != "config3":
+        w3 = make_workload("config3")
+        r3 = measure_device(B, w3, args, dev, order, loop, barrier, world)
+        r3["mesh"].destroy()
+        wet = (w3, r3)
+
+    vals = [ms, e2e_s * 1e3] + ([wet[1]["ms"]] if wet else [])
+    vals = max_over_ranks(vals, world, dev)
+    ms, e2e_ms = vals[0], vals[1]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -268,10 +313,13 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     value = job_throughput(n, args.steps, world, ms)
     peak, peak_src = load_peaks()
     kernel_ms = ms / args.steps                       # one step kernel launch per step
-    achieved = ALGO_BYTES_PER_CELL * n / (kernel_ms * 1e-3) / 1e9
-    traffic = load_traffic(args.workload)     # ncu dram bytes per launch of this workload (profiles/)
     sample, what = make_sample(args.workload)
     cpu_value, cpu_threads, _ = time_oracle(sample, 10 if sample.ncells > 300000 else 100, 2)
+
+    def l2_policy(cells):
+        return "inputs larger than L2 (no flush)" if cells * 164 > 2 * 126e6 \
+            else "working set fits in L2; a time loop re-reads its own output, no flush"
+
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -280,25 +328,12 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                    "ordering": args.ordering, "loop_mode": info["loop_mode"],
                    "grid": info["grid"], "block": info["block"], "tile_cells": tiles["tile_cells"],
                    "edge_evaluations_per_cell": round(tiles["edges_per_cell"], 4),
-                   "smem_bytes_per_block": tiles["smem_bytes"],
-                   "l2_policy": "inputs larger than L2 (no flush)" if n * 164 > 2 * 126e6
-                   else "working set fits in L2; a time loop re-reads its own output, no flush",
+                   "smem_bytes_per_block": tiles["smem_bytes"], "l2_policy": l2_policy(n),
                    "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "mesh_build_s": round(t_build, 2), "wet_fraction_end": 1.0 - stats["n_dry"] / n,
+                   "mesh_build_s": round(r["t_build"], 2), "wet_fraction_end": 1.0 - stats["n_dry"] / n,
                    "n_clamped": stats["n_clamped"]},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": traffic,
-                     # the same with 64 B (record in + out) for the cells of all-dry tiles, whose update
-                     # is the identity, and 156 B for the others
-                     "active_tile_share": active_share,
-                     "achieved_state_aware": (ALGO_BYTES_PER_CELL * active_share + 64.0 * (1.0 - active_share))
-                     * n / (kernel_ms * 1e-3) / 1e9,
-                     "frac_state_aware": (ALGO_BYTES_PER_CELL * active_share + 64.0 * (1.0 - active_share))
-                     * n / (kernel_ms * 1e-3) / 1e9 / peak,
-                     "achieved_dram": None if traffic is None else traffic / (kernel_ms * 1e-3) / 1e9,
-                     "frac_dram": None if traffic is None else traffic / (kernel_ms * 1e-3) / 1e9 / peak,
-                     "kernel": f"swe_step_kernel<{tiles['tile_cells']}>", "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
-                     "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0},
+        "roofline": roofline_record(n, kernel_ms, r["active_share"], r["list_share"], r["step_bytes"],
+                                    tiles, peak, peak_src),
         "cpu_baseline": {"value": cpu_value, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
                          "sample": what, "value_1_thread": getattr(time_oracle, "one_thread", None),
                          "host_cores": os.cpu_count()},
@@ -306,8 +341,20 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                 "h2d_bytes_per_step": 24.0 * n / args.steps, "d2h_bytes_per_step": 24.0 * n / args.steps,
                 "job": "swe_set_state(pinned host) + swe_run(K) + swe_get_state(pinned host); "
                        "bytes are per job / K"},
-        "gpu_launches": launches, "clocks": clocks,
+        "gpu_launches": r["launches"], "clocks": r["clocks"],
     }
+    if wet:
+        w3, r3 = wet
+        ms3 = vals[2]
+        line["wet"] = {
+            "workload": "config3", "name": w3.name, "cells": w3.ncells, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms3 / args.steps,
+            "value": job_throughput(w3.ncells, args.steps, world, ms3), "unit": UNIT,
+            "wet_fraction_end": 1.0 - r3["stats"]["n_dry"] / w3.ncells, "l2_policy": l2_policy(w3.ncells),
+            "grid": r3["info"]["grid"], "block": r3["info"]["block"], "gpu_launches": r3["launches"],
+            "roofline": roofline_record(w3.ncells, ms3 / args.steps, r3["active_share"], r3["list_share"],
+                                        r3["step_bytes"], r3["tiles"], peak, peak_src),
+        }
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -323,6 +370,8 @@ def main():
     ap.add_argument("--loop", default="auto", choices=["auto", "graph", "persistent", "launch"])
     ap.add_argument("--block", type=int, default=0, help="cells per tile = threads per block (0 = default)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-wet", dest="wet", action="store_false",
+                    help="skip the all-wet leg (config3) that the default run times beside the headline workload")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     rank = int(os.environ.get("RANK", "0"))

@@ -76,7 +76,7 @@ typedef struct {
 } swe_params;
 
 typedef struct {
-    double volume;        /* sum_i h_i |Omega_i| (m^3), summed on the host in long double */
+    double volume;        /* sum_i h_i |Omega_i| (m^3): fixed-tree partial sums on the device, added on the host */
     double t;             /* simulated time */
     double dt_last;       /* time step used by the most recent step (0 before the first) */
     int64_t steps;        /* steps taken since swe_set_state */
@@ -86,6 +86,9 @@ typedef struct {
     int64_t active_tile_steps; /* sum over the steps since swe_set_state of the number of tiles that were
                                   not all dry (tile + halo dry, no inflow edge: such tiles copy their
                                   records and skip the arithmetic) */
+    int64_t edge_list_fetches; /* sum over the steps of the number of tile edge lists read from HBM (the list of
+                                  a tile that was all dry at the previous step is read only if the tile turns
+                                  out active): with active_tile_steps it fixes the bytes a step requests */
 } swe_stats;
 
 /* Fills *p with the defaults listed above. */
@@ -221,6 +224,18 @@ int swe_get_tables(const swe_mesh *mesh, int32_t *nbr, double *normal, double *l
  */
 int swe_get_tile_info(const swe_mesh *mesh, int32_t *tile_cells, int64_t *ntiles, int64_t *nedges,
                       int32_t *max_edges, int32_t *max_halo, size_t *smem_bytes);
+
+/*
+ * Bytes one time step REQUESTS from device memory, from the library's own table sizes, given how
+ * many tiles are active (not all dry) and how many tile edge lists are fetched in that step (both
+ * may be per-step averages taken from swe_stats.active_tile_steps / edge_list_fetches): every cell's
+ * 32-byte record in and out, one 32-byte sector per halo record, tile headers + halo ids + hints,
+ * 24 bytes of cell constants per cell of an active tile, 24 bytes per edge of a fetched list (mean
+ * list length).  This is the kernel's request stream, not a DRAM counter: L2 hits on the halo
+ * records make the DRAM traffic smaller (bench.py reports it as roofline.traffic; the cross-check
+ * against ncu's dram__bytes is in profiles/).
+ */
+int swe_get_step_bytes(const swe_mesh *mesh, double active_tiles, double edge_lists, double *bytes);
 
 /*
  * The tile tables themselves, for tests of the mesh builder; any pointer may be NULL.

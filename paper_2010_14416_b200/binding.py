@@ -28,7 +28,7 @@ SYMBOLS = [
     "swe_compute_dt", "swe_step", "swe_run", "swe_run_until", "swe_get_boundary_volumes",
     "swe_snapshot_begin", "swe_snapshot_wait", "swe_sync", "swe_get_state", "swe_get_state_device",
     "swe_get_stats", "swe_get_permutation", "swe_get_tables", "swe_get_tile_info",
-    "swe_get_tile_tables", "swe_get_launch_info",
+    "swe_get_tile_tables", "swe_get_launch_info", "swe_get_step_bytes",
     "swe_last_error",
 ]
 
@@ -42,7 +42,8 @@ class SweParams(C.Structure):
 class SweStats(C.Structure):
     _fields_ = [("volume", C.c_double), ("t", C.c_double), ("dt_last", C.c_double),
                 ("steps", C.c_int64), ("n_dry", C.c_int64), ("n_clamped", C.c_int64),
-                ("n_nonfinite", C.c_int64), ("active_tile_steps", C.c_int64)]
+                ("n_nonfinite", C.c_int64), ("active_tile_steps", C.c_int64),
+                ("edge_list_fetches", C.c_int64)]
 
 
 class SweError(RuntimeError):
@@ -90,6 +91,7 @@ def load_library(rebuild_if_stale: bool = True):
                                     C.POINTER(C.c_size_t)]
     L.swe_get_tile_tables.argtypes = [vp, i32p, i32p, dp, i32p]
     L.swe_get_launch_info.argtypes = [vp, i32p, i32p, i32p, C.POINTER(C.c_int64)]
+    L.swe_get_step_bytes.argtypes = [vp, C.c_double, C.c_double, dp]
     L.swe_last_error.argtypes = [vp]
     L.swe_last_error.restype = C.c_char_p
     for name in SYMBOLS:
@@ -288,6 +290,11 @@ class SweMesh:
         self._ck(self._L.swe_get_tile_tables(self._h, a.ctypes.data_as(i32p), b.ctypes.data_as(i32p),
                                              _dp(geom), tinfo.ctypes.data_as(i32p)))
         return dict(edge_a=a, edge_b=b, edge_geom=geom, tinfo=tinfo, **ti)
+
+    def get_step_bytes(self, active_tiles, edge_lists) -> float:
+        b = C.c_double(0.0)
+        self._ck(self._L.swe_get_step_bytes(self._h, float(active_tiles), float(edge_lists), C.byref(b)))
+        return b.value
 
     def get_launch_info(self) -> dict:
         g, b, lm, n = C.c_int32(0), C.c_int32(0), C.c_int32(0), C.c_int64(0)

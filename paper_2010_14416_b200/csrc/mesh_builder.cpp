@@ -395,6 +395,7 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
             if (etot > (int64_t)INT32_MAX) { err = "too many edges"; return SWE_ERR_INVALID_ARG; }
             if (htot > (int64_t)INT32_MAX) { err = "too many halo cells"; return SWE_ERR_INVALID_ARG; }
             X.estart[(size_t)X.ntiles] = (int32_t)etot; hstart[(size_t)X.ntiles] = (int32_t)htot;
+            X.nhalo = htot;
             X.edges.resize((size_t)etot); halo.resize((size_t)htot);
             std::vector<std::thread> pool;
             for (Chunk &C : chunks) {

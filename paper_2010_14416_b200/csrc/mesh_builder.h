@@ -44,6 +44,7 @@ struct TileTables {
     int32_t max_edges = 0;             // longest (padded) edge list of any tile
     int64_t nedges = 0;                // edge records without the padding
     int32_t max_halo = 0;              // longest halo list of any tile, rounded up to a multiple of 4
+    int64_t nhalo = 0;                 // halo entries of all tiles together
     // [ntiles][4 + max_halo]: {first edge, #edges, #halo ids, 1 if the tile has an inflow edge else 0,
     // halo ids (internal cell ids of the tile's off-tile end points) padded with -1}
     std::vector<int32_t> tinfo;

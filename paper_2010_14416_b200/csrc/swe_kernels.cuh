@@ -68,6 +68,7 @@ struct Ctrl {                 // device-resident loop state
     long long steps;
     unsigned long long n_clamped;
     unsigned long long n_active;  // tiles that were not all dry, summed over the steps (diagnostics)
+    unsigned long long n_elists;  // edge lists fetched, summed over the steps (diagnostics)
     int all_dry;              // set when a step found no wet cell
     int bad_cell;             // smallest caller id with a negative depth or a non-finite value (swe_set_state)
 };
@@ -462,7 +463,7 @@ template <int TC>
 __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *smem,
                                              const Rec *__restrict__ Uin, Rec *__restrict__ Uout,
                                              const double dt, unsigned &nclamp, unsigned &nactive,
-                                             PipeState &ps)
+                                             unsigned &nelists, PipeState &ps)
 {
     typedef SmemLayout<TC> SL;
     constexpr int PLC = SL::PLC;
@@ -494,6 +495,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
         const unsigned bytes = (unsigned)((ne + 1) & ~1) * 24u;        // lists are padded to an even length
         mbar_expect_tx(bar + 2 + s, bytes);
         bulk_g2s(sedge0 + s * estride, P.edges + 3 * (size_t)e0, bytes, bar + 2 + s);
+        nelists++;
     };
     auto issue_cellc = [&](int t) {
         mbar_expect_tx(bar + 4, 3u * TC * 8u);

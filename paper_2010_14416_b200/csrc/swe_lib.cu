@@ -54,11 +54,12 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
         const double left = __ldcg(&P.ctrl->t_end) - t_now;
         const bool clipped = dt_cfl >= left;
         const double dt = fmax(clipped ? left : dt_cfl, 0.0);
-        unsigned nclamp = 0, nactive = 0;
-        double rate = step_tiles<TC>(P, dyn_smem, P.U(cur), P.U(cur ^ 1), dt, nclamp, nactive, it);
+        unsigned nclamp = 0, nactive = 0, nelists = 0;
+        double rate = step_tiles<TC>(P, dyn_smem, P.U(cur), P.U(cur ^ 1), dt, nclamp, nactive, nelists, it);
         rate = block_max(rate, s_red);
         if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
         if (nactive) atomicAdd(&P.ctrl->n_active, (unsigned long long)nactive);  // likewise (producer thread)
+        if (nelists) atomicAdd(&P.ctrl->n_elists, (unsigned long long)nelists);
         if (threadIdx.x == 0) {
             P.pmax(cur ^ 1)[blockIdx.x] = rate;
             if (blockIdx.x == 0) {
@@ -115,6 +116,37 @@ __global__ void swe_finalize_dt_kernel(const Params P, const int cur)
     __shared__ double s_red[32];
     const double dt = reduce_dt(P, P.pmax(cur), s_red);
     if (threadIdx.x == 0) P.ctrl->dt = dt;
+}
+
+// swe_get_stats on the device: per-block partial sums of h |Omega| (fixed tree, so the result does
+// not depend on timing), number of dry cells, number of non-finite cells.  out[block] = {volume,
+// dry, non-finite}; the host adds the <= kStatBlocks partials in block order.
+constexpr int kStatBlocks = 1024, kStatThreads = 256;
+struct StatPart { double volume; long long ndry, nbad; };
+__global__ void __launch_bounds__(kStatThreads)
+swe_stats_kernel(const Params P, const int cur, const int tile_cells, StatPart *__restrict__ out)
+{
+    __shared__ double s_v[kStatThreads];
+    __shared__ long long s_d[kStatThreads], s_b[kStatThreads];
+    double v = 0.0; long long nd = 0, nb = 0;
+    for (long long i = (long long)blockIdx.x * kStatThreads + threadIdx.x; i < P.nt; i += (long long)gridDim.x * kStatThreads) {
+        const Rec U = load_rec(P.U(cur) + i);
+        const int t = (int)(i / tile_cells), q = (int)(i - (long long)t * tile_cells);
+        const double area = 1.0 / __ldg(P.cellc + (size_t)t * 3 * tile_cells + q);
+        v += U.h * area;
+        nd += U.h <= P.hdry;
+        nb += !(isfinite(U.h) && isfinite(U.u) && isfinite(U.v));
+    }
+    s_v[threadIdx.x] = v; s_d[threadIdx.x] = nd; s_b[threadIdx.x] = nb;
+    __syncthreads();
+    for (int o = kStatThreads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+            s_v[threadIdx.x] += s_v[threadIdx.x + o]; s_d[threadIdx.x] += s_d[threadIdx.x + o];
+            s_b[threadIdx.x] += s_b[threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { out[blockIdx.x].volume = s_v[0]; out[blockIdx.x].ndry = s_d[0]; out[blockIdx.x].nbad = s_b[0]; }
 }
 
 // caller numbering (h, hu, hv) -> internal records {h, u, v, z}; dry cells lose their momentum
@@ -259,6 +291,9 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
 int swe_mesh_destroy(swe_mesh *m)
 {
     if (!m) return SWE_OK;
+    // steps still queued on the stream write the caller's workspace: let them finish before the
+    // caller is told it may free or reuse that memory
+    if (m->bound) cudaStreamSynchronize(m->stream);
     for (auto &kv : m->graphs) cudaGraphExecDestroy(kv.second);
     if (m->snap_pending) cudaEventSynchronize(m->ev_done);
     if (m->ev_ready) cudaEventDestroy(m->ev_ready);
@@ -307,6 +342,22 @@ int swe_get_tile_info(const swe_mesh *m, int32_t *tile_cells, int64_t *ntiles, i
     if (max_edges) *max_edges = m->X.max_edges;
     if (max_halo) *max_halo = m->X.max_halo;
     if (smem_bytes) *smem_bytes = tile_smem_bytes(m->X.tile_cells, m->X.max_halo, m->X.max_edges);
+    return SWE_OK;
+}
+
+int swe_get_step_bytes(const swe_mesh *m, double active_tiles, double edge_lists, double *bytes)
+{
+    if (!m || !bytes || !(active_tiles >= 0.0) || !(edge_lists >= 0.0)) return SWE_ERR_INVALID_ARG;
+    const TileTables &X = m->X;
+    const double nt = (double)m->T.nt, ntiles = (double)X.ntiles, TC = (double)X.tile_cells;
+    double b = 0.0;
+    b += 32.0 * nt;                                   // every cell's record read (TMA bulk copy) ...
+    b += 32.0 * nt;                                   // ... and written (256-bit store)
+    b += 32.0 * (double)X.nhalo;                      // halo records, one 32-byte sector each
+    b += ntiles * (16.0 + 4.0 * (double)std::min(X.max_halo, X.tile_cells) + 8.0);  // header, halo ids, hint in and out
+    b += active_tiles * 24.0 * TC;                    // cell constants of the tiles that are not all dry
+    b += edge_lists * 24.0 * (double)X.edges.size() / ntiles;   // edge lists fetched (mean list length)
+    *bytes = b;
     return SWE_OK;
 }
 
@@ -369,6 +420,10 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     const TileTables &X = m->X;
     m->smem = tile_smem_bytes(m->block, X.max_halo, X.max_edges);
     if (m->smem > (size_t)smem_optin - 1024) { m->err = "tile does not fit in shared memory"; return SWE_ERR_CUDA; }
+    // end point words hold 13-bit positions, tile headers 12-bit counts (swe_kernels.cuh)
+    if (m->block + X.max_halo > (int)kPosMask || X.max_edges > 4095 || X.max_halo > 4095) {
+        m->err = "tile edge / halo lists too long for the kernel's tables"; return SWE_ERR_INVALID_ARG;
+    }
     m->kern = step_kernel_for(m->block);
     // the attribute belongs to the kernel, not to this handle: allow the device maximum so that
     // handles with different tile tables can coexist
@@ -517,7 +572,9 @@ int swe_compute_dt(swe_mesh *m, double *dt_out)
     if (!m) return SWE_ERR_INVALID_ARG;
     if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
     if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
-    m->have_rates = false;      // recompute from the current state, as documented
+    // the per-block maxima of the current state are already on the device after a step (the step
+    // kernel leaves them for the next one); recomputing them here with another kernel could differ
+    // in the last bit and make a run depend on whether this getter was called
     Ctrl c;
     int rc = read_ctrl(m, &c, true);
     if (rc != SWE_OK) return rc;
@@ -739,23 +796,24 @@ int swe_get_stats(swe_mesh *m, swe_stats *s)
     if (!m || !s) return SWE_ERR_INVALID_ARG;
     if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
     if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
-    const size_t n = (size_t)m->T.nt;
-    std::vector<double> h(n), hu(n), hv(n);
-    double t = 0;
-    int rc = swe_get_state(m, h.data(), hu.data(), hv.data(), &t, nullptr);
+    int rc = snapshot_finish(m);       // the partial sums live in the staging buffer
     if (rc != SWE_OK) return rc;
+    const int nblk = (int)std::min<int64_t>(kStatBlocks, (m->T.nt + kStatThreads - 1) / kStatThreads);
+    StatPart *d_part = reinterpret_cast<StatPart *>(m->d_stage);
+    swe_stats_kernel<<<nblk, kStatThreads, 0, m->stream>>>(m->P, m->cur, m->X.tile_cells, d_part);
+    m->launches++;
+    CK(cudaGetLastError());
+    std::vector<StatPart> part((size_t)nblk);
+    CK(cudaMemcpyAsync(part.data(), d_part, sizeof(StatPart) * (size_t)nblk, cudaMemcpyDeviceToHost, m->stream));
     Ctrl c;
-    rc = read_ctrl(m, &c, false);
+    rc = read_ctrl(m, &c, false);      // synchronises the stream
     if (rc != SWE_OK) return rc;
     long double vol = 0.0L; int64_t ndry = 0, nbad = 0;
-    for (size_t i = 0; i < n; i++) {
-        vol += (long double)h[i] * (long double)m->T.area[i];
-        ndry += h[i] <= m->prm.h_dry;
-        nbad += !(std::isfinite(h[i]) && std::isfinite(hu[i]) && std::isfinite(hv[i]));
-    }
+    for (const StatPart &p : part) { vol += (long double)p.volume; ndry += p.ndry; nbad += p.nbad; }
     s->volume = (double)vol; s->t = c.t[m->cur]; s->dt_last = c.dt_last; s->steps = c.steps;
     s->n_dry = ndry; s->n_clamped = (int64_t)c.n_clamped; s->n_nonfinite = nbad;
     s->active_tile_steps = (int64_t)c.n_active;
+    s->edge_list_fetches = (int64_t)c.n_elists;
     return SWE_OK;
 }
 

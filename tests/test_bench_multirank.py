@@ -54,3 +54,19 @@ def test_reference_arm_under_torchrun_prints_one_line():
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0,
                         "d2h_bytes_per_step": 0}
     assert d["config"]["workload"] == "config1" and d["dtype"] == "f64"
+
+
+def test_roofline_record_is_reproducible_from_its_own_fields():
+    """roofline.frac = (156 B x cells of active tiles + 64 B x cells of all-dry tiles) / time / peak:
+    it can be recomputed by hand from the line, and skipping work (a low active share) lowers the
+    bytes it is credited with instead of inflating the fraction."""
+    import bench
+    tiles = {"tile_cells": 192}
+    n, ms, peak = 13_005_000, 0.2, 6547.5
+    r = bench.roofline_record(n, ms, 0.063, 0.07, 9.0e8, tiles, peak, "test")
+    algo = (156.0 * 0.063 + 64.0 * (1 - 0.063)) * n
+    assert r["achieved"] == algo / (ms * 1e-3) / 1e9 and r["frac"] == r["achieved"] / peak
+    assert r["frac"] < 1.0 < r["frac_fixed_156"]            # the round-1 headline (1.53) was this one
+    assert r["traffic"] == 9.0e8 and r["frac_traffic"] == 9.0e8 / (ms * 1e-3) / 1e9 / peak
+    full = bench.roofline_record(n, ms, 1.0, 1.0, 9.0e8, tiles, peak, "test")
+    assert full["frac"] == full["frac_fixed_156"]
