@@ -191,6 +191,69 @@ def test_device_state_roundtrip():
     np.testing.assert_array_equal(out[2].cpu().numpy(), hv)
 
 
+def test_clockwise_input_and_permuted_tags_on_the_device():
+    """Every other triangle given clockwise with its edge tags permuted accordingly (river case:
+    inflow, outflow, walls, bed, friction): the device run matches the oracle on the same flipped
+    input, and is bit-identical to the run on the counter-clockwise input."""
+    w = W.config4(nx=240, ny=60)
+    f = W.config4(nx=240, ny=60)
+    flip = np.arange(w.ncells) % 2 == 0
+    f.tris[flip] = f.tris[flip][:, [0, 2, 1]]
+    f.bc_tags[flip] = f.bc_tags[flip][:, [2, 1, 0]]
+    m, o = run_both(f, 400)
+    got = assert_parity(m, o, f)
+    r = B.SweMesh.from_workload(w).bind_device()
+    r.set_state(w.h, w.hu, w.hv)
+    r.run(400)
+    for a, b in zip(got[:3], r.get_state()[:3]):
+        np.testing.assert_array_equal(a, b)
+    np.testing.assert_array_equal(m.get_boundary_volumes(), r.get_boundary_volumes())
+
+
+def test_eq22_clamp_branch_strongly_diverging_flow():
+    """R-6: two halves of a canal moving apart at |u| = 15 m/s with h = 1 m (u_R - u_L > 8 a, so
+    the bracket of eq.(22) is negative and its unclamped square would exceed h_k): the edges along
+    the parting line take the clamped branch on both sides; a dry bed opens between them."""
+    w = W.canal_dam_break(120, 12, h_left=1.0, h_right=1.0, manning=0.02, length=120.0, seed=77)
+    w.bc_tags[w.bc_tags > 0] = W.BC_TRANSMISSIVE
+    cx = W.centroids(w.nodes_xy, w.tris)[:, 0]
+    w.hu[:] = np.where(cx < 60.0, -15.0, 15.0) * w.h
+    assert 30.0 > 8.0 * np.sqrt(9.81 * 1.0)
+    from oracle.swe_oracle import hllc
+    assert hllc(1.0, -15.0, 0.0, 1.0, 15.0, 0.0)[1]["hs"] == 0.0        # the branch in question
+    m, o = run_both(w, 60)
+    h, hu, hv, t = assert_parity(m, o, w)
+    assert h.min() < 0.2 and (np.abs(hu) > 1.0).any()                   # the bed is emptying at the parting line
+
+
+def test_dry_inflow_cells():
+    """R-20, dry branch: the whole left edge is an inflow boundary, including the dry floodplain
+    cells, which receive the mass flux q_n and no momentum flux while they are dry."""
+    w = W.config4(nx=480, ny=120)
+    cx = W.centroids(w.nodes_xy, w.tris)[:, 0]
+    for k in range(3):
+        xa = w.nodes_xy[w.tris[:, k], 0]
+        xb = w.nodes_xy[w.tris[:, (k + 1) % 3], 0]
+        w.bc_tags[(xa == 0.0) & (xb == 0.0), k] = W.BC_INFLOW0
+    left = (w.bc_tags == W.BC_INFLOW0).any(axis=1)
+    assert (w.h[left] <= w.h_dry).any() and (w.h[left] > w.h_dry).any()
+    m, o = run_both(w, 500)
+    h, hu, hv, t = assert_parity(m, o, w)
+    assert (h[left] > w.h_dry).all()                                     # the dry inflow cells have filled
+    vg, vo = m.get_boundary_volumes(), o.boundary_volumes()
+    np.testing.assert_allclose(vg, vo, rtol=1e-10, atol=1e-10)
+    assert vg[W.BC_INFLOW0] == pytest.approx(-500.0 * t, rel=1e-12)
+
+
+@pytest.mark.parametrize("ordering", [B.ORDER_IDENTITY, B.ORDER_HILBERT])
+def test_config5_sweep_2M_both_orderings(ordering):
+    """BASELINE configs[4], the 2M-cell sweep mesh (1,997,120 cells), all 200 steps, with the
+    caller's random numbering kept and with the Hilbert renumbering: every cell against the oracle."""
+    w = W.config5("2M")
+    m, o = run_both(w, w.nsteps, ordering=ordering)
+    assert_parity(m, o, w)
+
+
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times (defaults) ----------
 def test_config3_full_size_every_cell_then_invariants():
     """configs[2] at 2000x1000 squares (4,000,000 cells): every cell against the oracle after 40

@@ -85,8 +85,16 @@ def test_clockwise_triangles_and_tag_permutation():
     a = B.SweMesh(w.nodes_xy, w.tris, w.bathymetry, w.manning, w.bc_tags).get_tables()
     b = B.SweMesh(w.nodes_xy, tris, w.bathymetry, w.manning, tags).get_tables()
     # an unflipped cell is unchanged; a flipped cell (v0,v2,v1) is re-oriented to (v0,v1,v2)
-    for key in ("nbr", "length", "area", "inradius"):
+    # (nbr holds -tag on boundary edges, so the permuted tags must have landed on the right edges)
+    for key in ("nbr", "length", "area", "inradius", "normal", "cell_z"):
         np.testing.assert_array_equal(a[key], b[key])
+    assert (a["nbr"] < 0).any() and (a["nbr"] == -W.BC_INFLOW0).any() and (a["nbr"] == -W.BC_TRANSMISSIVE).any()
+    # and against the oracle's own orientation fix on the flipped input
+    from oracle.swe_oracle import OracleSolver
+    geo = OracleSolver(w.nodes_xy, tris, w.bathymetry, w.manning, tags).geometry()
+    np.testing.assert_allclose(b["normal"][:, :, 0], geo["n1"], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(b["normal"][:, :, 1], geo["n2"], rtol=0, atol=1e-15)
+    np.testing.assert_array_equal(np.where(b["nbr"] >= 0, b["nbr"], -1), geo["nbr"])
 
 
 def test_invalid_input_codes():
