@@ -49,7 +49,9 @@ typedef enum {
     SWE_ERR_ALL_DRY = -9,       /* every cell is dry: no time step can be defined */
     SWE_ERR_NO_STATE = -10,     /* swe_set_state has not been called */
     SWE_ERR_BAD_TAG = -11,      /* boundary tag out of range or without edges */
-    SWE_ERR_NOMEM = -12
+    SWE_ERR_NOMEM = -12,
+    SWE_ERR_IO = -13,           /* a mesh file cannot be opened */
+    SWE_ERR_FORMAT = -14        /* a mesh file does not follow the layout of PAPER.md Fig. 4 */
 } swe_status;
 
 /* boundary tags of bc_tags */
@@ -112,6 +114,21 @@ int swe_params_default(swe_params *p);
 int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_t nt,
                     const double *bathymetry, const double *manning, const int8_t *bc_tags,
                     const swe_params *params, swe_mesh **out);
+
+/*
+ * Reads a mesh file in the paper's layout (Fig. 4): a title line, the number of
+ * nodes on its own line, one row "id x y z" per node; a title line, the number of cells, one row
+ * "id n1 n2 n3 manning" per cell.  Ids are 1-based in the file and 0-based in the arrays; rows may
+ * come in any order.  What follows the connectivity table (the "Ghost cells to be sent / received"
+ * block lists of the paper's multi-GPU decomposition) is ignored.  The file carries no boundary
+ * tags (the paper flags inflow nodes separately): pass your own bc_tags to
+ * swe_mesh_create, or zeros for solid walls.
+ * Call once with all four arrays NULL to get *nn and *nt, allocate, call again:
+ *   nodes_xy host [nn][2], bathymetry host [nn], tris host [nt][3], manning host [nt] (any may be NULL)
+ * Errors: SWE_ERR_IO, SWE_ERR_FORMAT (message with the line number in swe_last_error(NULL)).
+ */
+int swe_mesh_file_read(const char *path, int64_t *nn, int64_t *nt, double *nodes_xy,
+                       double *bathymetry, int32_t *tris, double *manning);
 
 /* Frees the host tables and CUDA graphs.  Never frees the caller's device workspace. */
 int swe_mesh_destroy(swe_mesh *mesh);

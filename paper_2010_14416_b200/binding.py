@@ -23,7 +23,7 @@ ERR_ALL_DRY = -9
 
 # every symbol include/swe.h declares
 SYMBOLS = [
-    "swe_params_default", "swe_mesh_create", "swe_mesh_destroy", "swe_mesh_workspace_bytes",
+    "swe_params_default", "swe_mesh_create", "swe_mesh_file_read", "swe_mesh_destroy", "swe_mesh_workspace_bytes",
     "swe_mesh_bind_device", "swe_set_bc_value", "swe_set_state", "swe_set_state_device",
     "swe_compute_dt", "swe_step", "swe_run", "swe_run_until", "swe_get_boundary_volumes",
     "swe_snapshot_begin", "swe_snapshot_wait", "swe_sync", "swe_get_state", "swe_get_state_device",
@@ -68,6 +68,7 @@ def load_library(rebuild_if_stale: bool = True):
     L.swe_params_default.argtypes = [C.POINTER(SweParams)]
     L.swe_mesh_create.argtypes = [dp, i64, i32p, i64, dp, dp, C.POINTER(C.c_int8),
                                   C.POINTER(SweParams), C.POINTER(vp)]
+    L.swe_mesh_file_read.argtypes = [C.c_char_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), dp, dp, i32p, dp]
     L.swe_mesh_destroy.argtypes = [vp]
     L.swe_mesh_workspace_bytes.argtypes = [vp, C.POINTER(C.c_size_t)]
     L.swe_mesh_bind_device.argtypes = [vp, vp, C.c_size_t, vp]
@@ -103,6 +104,24 @@ def load_library(rebuild_if_stale: bool = True):
 
 def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double)) if a is not None else None
+
+
+def read_mesh_file(path):
+    """Mesh file in the paper's layout (Fig. 4) -> dict of 0-based arrays
+    (nodes_xy, bathymetry, tris, manning); the file has no boundary tags."""
+    L = load_library()
+    nn, nt = C.c_int64(0), C.c_int64(0)
+    enc = os.fsencode(path)
+    rc = L.swe_mesh_file_read(enc, C.byref(nn), C.byref(nt), None, None, None, None)
+    if rc != 0:
+        raise SweError(rc, (L.swe_last_error(None) or b"").decode())
+    xy, z = np.empty((nn.value, 2)), np.empty(nn.value)
+    tris, mn = np.empty((nt.value, 3), dtype=np.int32), np.empty(nt.value)
+    rc = L.swe_mesh_file_read(enc, C.byref(nn), C.byref(nt), _dp(xy), _dp(z),
+                              tris.ctypes.data_as(C.POINTER(C.c_int32)), _dp(mn))
+    if rc != 0:
+        raise SweError(rc, (L.swe_last_error(None) or b"").decode())
+    return dict(nodes_xy=xy, bathymetry=z, tris=tris, manning=mn)
 
 
 class SweMesh:

@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <numeric>
 #include <atomic>
 #include <new>
@@ -260,6 +261,91 @@ int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_
     else if (ordering == SWE_ORDER_RCM) order_rcm(T);
     else std::iota(T.perm.begin(), T.perm.end(), 0);
     for (int64_t p = 0; p < nt; p++) T.inv[(size_t)T.perm[(size_t)p]] = (int32_t)p;
+    return SWE_OK;
+}
+
+// ---- the paper's mesh file (Fig. 4) ---------------------------------------------
+namespace {
+// splits a line into numeric tokens; returns false if a token is not a number (a title line)
+bool numeric_tokens(const char *line, std::vector<double> &tok)
+{
+    tok.clear();
+    const char *p = line;
+    for (;;) {
+        while (*p == ' ' || *p == '\t' || *p == '\r' || *p == '\n' || *p == ',' || *p == '|') p++;
+        if (!*p) return true;
+        char *end = nullptr;
+        const double v = std::strtod(p, &end);
+        if (end == p) return false;
+        if (*end && *end != ' ' && *end != '\t' && *end != '\r' && *end != '\n' && *end != ',' && *end != '|') return false;
+        tok.push_back(v);
+        p = end;
+    }
+}
+} // namespace
+
+int read_mesh_file(const char *path, int64_t *nn_out, int64_t *nt_out, double *nodes_xy, double *bathymetry,
+                   int32_t *tris, double *manning, std::string &err)
+{
+    if (!path || !nn_out || !nt_out) { err = "read_mesh_file: NULL argument"; return SWE_ERR_INVALID_ARG; }
+    FILE *f = std::fopen(path, "r");
+    if (!f) { err = std::string("cannot open mesh file ") + path; return SWE_ERR_IO; }
+    const bool fill = nodes_xy || bathymetry || tris || manning;
+    std::vector<char> buf(1 << 16);
+    std::vector<double> tok;
+    std::vector<unsigned char> seen;
+    int64_t count[2] = { -1, -1 }, rows = 0, lineno = 0;
+    int table = -1;                 // 0 node table, 1 connectivity table; -1 before the first count
+    int rc = SWE_OK;
+    auto fail = [&](const std::string &what) {
+        err = std::string(path) + ":" + std::to_string(lineno) + ": " + what; rc = SWE_ERR_FORMAT;
+    };
+    while (rc == SWE_OK && std::fgets(buf.data(), (int)buf.size(), f)) {
+        lineno++;
+        if (!numeric_tokens(buf.data(), tok)) {                // a title line
+            if (table == 1 && rows == count[1]) break;          // "Ghost cells ...": the rest is multi-GPU
+            if (table >= 0 && rows < count[table]) { fail("text inside a table"); break; }
+            continue;
+        }
+        if (tok.empty()) continue;
+        if (table < 0 || (rows == count[table] && table == 0)) {   // the count line that opens a table
+            if (tok.size() != 1 || tok[0] < 1.0 || tok[0] != std::floor(tok[0]) || tok[0] >= 2147483647.0) {
+                fail("expected the number of rows on its own line"); break;
+            }
+            table++; count[table] = (int64_t)tok[0]; rows = 0;
+            if (fill) seen.assign((size_t)count[table], 0);
+            continue;
+        }
+        if (rows == count[table]) break;                        // numbers after the connectivity table: ghost lists
+        const size_t want = table == 0 ? 4 : 5;
+        if (tok.size() != want) { fail(table == 0 ? "a node row is: id x y z" : "a cell row is: id n1 n2 n3 manning"); break; }
+        const double idd = tok[0];
+        if (idd < 1.0 || idd > (double)count[table] || idd != std::floor(idd)) { fail("row id out of range (ids are 1-based)"); break; }
+        const size_t i = (size_t)idd - 1;
+        if (fill) {
+            if (seen[i]) { fail("row id appears twice"); break; }
+            seen[i] = 1;
+            if (table == 0) {
+                if (nodes_xy) { nodes_xy[2 * i] = tok[1]; nodes_xy[2 * i + 1] = tok[2]; }
+                if (bathymetry) bathymetry[i] = tok[3];
+            } else {
+                for (int k = 0; k < 3; k++) {
+                    const double v = tok[1 + k];
+                    if (v < 1.0 || v > (double)count[0] || v != std::floor(v)) { fail("node id out of range (ids are 1-based)"); break; }
+                    if (tris) tris[3 * i + k] = (int32_t)v - 1;
+                }
+                if (manning) manning[i] = tok[4];
+            }
+        }
+        rows++;
+    }
+    std::fclose(f);
+    if (rc != SWE_OK) return rc;
+    if (count[0] < 0 || count[1] < 0 || rows != count[1]) {
+        err = std::string(path) + ": truncated (node table, then connectivity table expected)";
+        return SWE_ERR_FORMAT;
+    }
+    *nn_out = count[0]; *nt_out = count[1];
     return SWE_OK;
 }
 

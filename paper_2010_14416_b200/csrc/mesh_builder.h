@@ -64,6 +64,14 @@ constexpr uint32_t kDevPosMask = 0x1FFFu, kDevNoSlot = 0x7FFFu;
 constexpr int kDevKShift = 13, kDevSlotShift = 16;
 void pack_device_edges(const TileTables &X, std::vector<double> &out);
 
+// Reader for the paper's mesh-file layout (Fig. 4): a node table (a title line, the
+// node count on its own line, rows "id x y z") and a connectivity table (title, cell count, rows
+// "id n1 n2 n3 manning"), ids 1-based; anything after the connectivity rows (the "Ghost cells to be
+// sent / received" block lists of the multi-GPU decomposition) is ignored.  With all array pointers
+// NULL only the counts are returned.  Returns SWE_OK or a negative swe_status with a message in err.
+int read_mesh_file(const char *path, int64_t *nn, int64_t *nt, double *nodes_xy, double *bathymetry,
+                   int32_t *tris, double *manning, std::string &err);
+
 // Returns SWE_OK or a negative swe_status with a message in err.
 int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, std::string &err);
 

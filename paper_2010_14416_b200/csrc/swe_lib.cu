@@ -288,6 +288,14 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     return SWE_OK;
 }
 
+int swe_mesh_file_read(const char *path, int64_t *nn, int64_t *nt, double *nodes_xy,
+                       double *bathymetry, int32_t *tris, double *manning)
+{
+    try {
+        return read_mesh_file(path, nn, nt, nodes_xy, bathymetry, tris, manning, g_create_err);
+    } catch (const std::bad_alloc &) { g_create_err = "out of host memory"; return SWE_ERR_NOMEM; }
+}
+
 int swe_mesh_destroy(swe_mesh *m)
 {
     if (!m) return SWE_OK;

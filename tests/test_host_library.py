@@ -193,3 +193,55 @@ def test_tile_tables_cover_every_cell_edge_exactly_once(ordering, block):
     if ordering == B.ORDER_HILBERT and block >= 192:
         assert X["edges_per_cell"] < 1.85
     assert 1.5 <= X["edges_per_cell"] <= 3.0
+
+
+# ------------------------------------------------------------------ the paper's mesh file (Fig. 4)
+def test_mesh_file_reader_hand_written_file():
+    """PAPER.md:296-328 Fig. 4: node table "id x y z", connectivity table "id n1 n2 n3 manning",
+    counts on their own lines, 1-based ids, ghost-block sections (multi-GPU) ignored.  The
+    hand-written 4-node file is the two-triangle mesh of workloads.two_triangles()."""
+    import os
+    d = B.read_mesh_file(os.path.join(os.path.dirname(__file__), "golden", "fig4_two_triangles.txt"))
+    w = W.two_triangles()
+    np.testing.assert_array_equal(d["nodes_xy"], w.nodes_xy)
+    np.testing.assert_array_equal(d["tris"], w.tris)
+    np.testing.assert_array_equal(d["bathymetry"], [0.25, 0.5, 0.75, 1.0])     # rows 3 and 4 are swapped in the file
+    np.testing.assert_array_equal(d["manning"], [0.03, 0.05])
+    # feeds swe_mesh_create as it is (no tags in the file: walls)
+    m = B.SweMesh(d["nodes_xy"], d["tris"], d["bathymetry"], d["manning"], np.zeros((2, 3), dtype=np.int8))
+    t = m.get_tables()
+    np.testing.assert_allclose(t["area"], [0.5, 0.5], rtol=1e-15)
+    np.testing.assert_allclose(t["cell_z"], [0.5, 2.0 / 3.0], rtol=1e-15)
+
+
+def test_mesh_file_reader_round_trip_and_errors(tmp_path):
+    w = W.config4(nx=30, ny=8)
+    p = tmp_path / "mesh.txt"
+    with open(p, "w") as f:
+        f.write("Coordinate table\n%d\n" % w.nnodes)
+        for i in range(w.nnodes):
+            f.write("%d %.17g %.17g %.17g\n" % (i + 1, w.nodes_xy[i, 0], w.nodes_xy[i, 1], w.bathymetry[i]))
+        f.write("Connectivity table\n%d\n" % w.ncells)
+        for i in range(w.ncells):
+            f.write("%d %d %d %d %.17g\n" % (i + 1, w.tris[i, 0] + 1, w.tris[i, 1] + 1, w.tris[i, 2] + 1, w.manning[i]))
+    d = B.read_mesh_file(str(p))
+    np.testing.assert_array_equal(d["nodes_xy"], w.nodes_xy)
+    np.testing.assert_array_equal(d["bathymetry"], w.bathymetry)
+    np.testing.assert_array_equal(d["tris"], w.tris)
+    np.testing.assert_array_equal(d["manning"], w.manning)
+    with pytest.raises(B.SweError) as e:
+        B.read_mesh_file(str(tmp_path / "missing.txt"))
+    assert e.value.code == -13
+    bad = tmp_path / "bad.txt"
+    bad.write_text("Coordinate table\n2\n1 0 0 0\n3 1 0 0\n")          # id 3 of 2
+    with pytest.raises(B.SweError) as e:
+        B.read_mesh_file(str(bad))
+    assert e.value.code == -14 and ":4:" in str(e.value)
+    bad.write_text("Coordinate table\n2\n1 0 0 0\n2 1 0 0\nConnectivity table\n1\n1 1 2 5 0.03\n")   # node 5 of 2
+    with pytest.raises(B.SweError) as e:
+        B.read_mesh_file(str(bad))
+    assert e.value.code == -14
+    bad.write_text("Coordinate table\n2\n1 0 0 0\n2 1 0 0\nConnectivity table\n2\n1 1 2 2 0.03\n")   # truncated
+    with pytest.raises(B.SweError) as e:
+        B.read_mesh_file(str(bad))
+    assert e.value.code == -14
