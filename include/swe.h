@@ -61,6 +61,14 @@ enum { SWE_ORDER_IDENTITY = 0, SWE_ORDER_HILBERT = 1, SWE_ORDER_RCM = 2 };
 /* swe_params.riemann: HLLC (the paper's scheme) or plain HLL for all three
  * components (eq.17-18) */
 enum { SWE_RIEMANN_HLLC = 0, SWE_RIEMANN_HLL = 1 };
+/* swe_params.kernel: TILED = the fused tile kernel (one launch per step: every edge of a tile once in
+ * shared memory, then the tile's cells); EDGE_TWO_PASS = the edge-centric alternative the paper's text
+ * leaves open: pass 1, one thread per edge of the mesh, writes the edge's
+ * length-weighted flux + sources for both sides to HBM; pass 2, one thread per cell, adds its three
+ * edges in the order k = 0,1,2 and does friction, update and rate.  Same arithmetic, same results;
+ * more HBM traffic, no shared-memory scatter (A/B in profiles/).  No dry-tile shortcut, GRAPH or
+ * LAUNCH loop only. */
+enum { SWE_KERNEL_TILED = 0, SWE_KERNEL_EDGE_TWO_PASS = 1 };
 /* swe_params.loop_mode: how swe_run iterates without host round trips: GRAPH = CUDA graphs of
  * 128 / 16 / 2 step-kernel launches, PERSISTENT = one cooperative launch with a grid barrier per
  * step, LAUNCH = plain launches; AUTO = GRAPH (measured as fast or faster at every mesh size) */
@@ -75,6 +83,8 @@ typedef struct {
     int32_t block_size; /* cells per tile = CUDA threads per block: 64, 128, 192 or 256; 0 = default (192) */
     int32_t loop_mode;  /* SWE_LOOP_*; default SWE_LOOP_AUTO */
     int32_t riemann;    /* SWE_RIEMANN_*; default SWE_RIEMANN_HLLC */
+    int32_t kernel;     /* SWE_KERNEL_*; default SWE_KERNEL_TILED */
+    int32_t reserved;   /* 0 */
 } swe_params;
 
 typedef struct {

@@ -18,6 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 ORDER_IDENTITY, ORDER_HILBERT, ORDER_RCM = 0, 1, 2
 LOOP_AUTO, LOOP_GRAPH, LOOP_PERSISTENT, LOOP_LAUNCH = 0, 1, 2, 3
 RIEMANN_HLLC, RIEMANN_HLL = 0, 1
+KERNEL_TILED, KERNEL_EDGE_TWO_PASS = 0, 1
 LOOP_NAMES = {0: "auto", 1: "graph", 2: "persistent", 3: "launch"}
 ERR_ALL_DRY = -9
 
@@ -36,7 +37,7 @@ SYMBOLS = [
 class SweParams(C.Structure):
     _fields_ = [("g", C.c_double), ("cfl", C.c_double), ("h_dry", C.c_double),
                 ("ordering", C.c_int32), ("block_size", C.c_int32), ("loop_mode", C.c_int32),
-                ("riemann", C.c_int32)]
+                ("riemann", C.c_int32), ("kernel", C.c_int32), ("reserved", C.c_int32)]
 
 
 class SweStats(C.Structure):
@@ -129,7 +130,7 @@ class SweMesh:
 
     def __init__(self, nodes_xy, tris, bathymetry, manning, bc_tags, *, g=9.81, cfl=0.9,
                  h_dry=1e-6, ordering=ORDER_HILBERT, block_size=0, loop_mode=LOOP_AUTO,
-                 riemann=RIEMANN_HLLC):
+                 riemann=RIEMANN_HLLC, kernel=KERNEL_TILED):
         self._h = None
         L = load_library()
         self._L = L
@@ -147,6 +148,7 @@ class SweMesh:
         p.g, p.cfl, p.h_dry = float(g), float(cfl), float(h_dry)
         p.ordering, p.block_size, p.loop_mode = int(ordering), int(block_size), int(loop_mode)
         p.riemann = int(riemann)
+        p.kernel = int(kernel)
         self.params = p
         h = C.c_void_p()
         rc = L.swe_mesh_create(_dp(xy), self.nn, tr.ctypes.data_as(C.POINTER(C.c_int32)), self.nt,

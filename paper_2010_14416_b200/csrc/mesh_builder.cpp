@@ -264,6 +264,49 @@ int build_tables(const double *nodes_xy, int64_t nn, const int32_t *tris, int64_
     return SWE_OK;
 }
 
+// ---- global edge list of the edge-centric two-pass kernels ----------------------------------------
+int build_global_edges(const HostTables &T, GlobalEdges &E, std::string &err)
+{
+    const int64_t nt = T.nt;
+    try {
+        E.edges.clear(); E.edges.reserve((size_t)nt * 3 / 2 + 1024);
+        E.cedge.assign(3 * (size_t)nt, -1);
+        std::vector<int32_t> bnum(3 * (size_t)nt, -1);          // boundary edges in (caller cell, local edge) order
+        int32_t nb = 0;
+        for (size_t e = 0; e < 3 * (size_t)nt; e++) if (T.nbr[e] < 0) bnum[e] = nb++;
+        for (int64_t p = 0; p < nt; p++) {
+            const int32_t c = T.perm[(size_t)p];
+            for (int k = 0; k < 3; k++) {
+                const int32_t j = T.nbr[3 * (size_t)c + k];
+                const double L = T.length[3 * (size_t)c + k];
+                const double *nk = &T.normal[6 * (size_t)c + 2 * k];
+                if (E.edges.size() >= (size_t)1 << 30) { err = "too many edges"; return SWE_ERR_INVALID_ARG; }
+                const int32_t id = (int32_t)E.edges.size();
+                if (j < 0) {
+                    E.edges.push_back({ (int32_t)p, -((-j) + 128 * bnum[3 * (size_t)c + k]), L * nk[0], L * nk[1] });
+                    E.cedge[3 * (size_t)p + k] = 2 * id;
+                    continue;
+                }
+                const int64_t pj = T.inv[(size_t)j];
+                if (pj < p) continue;                            // emitted when pj was visited
+                int kj = -1;
+                for (int q = 0; q < 3; q++) if (T.nbr[3 * (size_t)j + q] == c) kj = q;
+                if (kj < 0) { err = "inconsistent neighbour table"; return SWE_ERR_NON_MANIFOLD; }
+                if (c < j) {                                     // a = smaller caller id (R-17)
+                    E.edges.push_back({ (int32_t)p, (int32_t)pj, L * nk[0], L * nk[1] });
+                    E.cedge[3 * (size_t)p + k] = 2 * id; E.cedge[3 * (size_t)pj + kj] = 2 * id + 1;
+                } else {
+                    const double Lj = T.length[3 * (size_t)j + kj];
+                    E.edges.push_back({ (int32_t)pj, (int32_t)p, Lj * T.normal[6 * (size_t)j + 2 * kj],
+                                        Lj * T.normal[6 * (size_t)j + 2 * kj + 1] });
+                    E.cedge[3 * (size_t)pj + kj] = 2 * id; E.cedge[3 * (size_t)p + k] = 2 * id + 1;
+                }
+            }
+        }
+    } catch (const std::bad_alloc &) { err = "out of host memory"; return SWE_ERR_NOMEM; }
+    return SWE_OK;
+}
+
 // ---- the paper's mesh file (Fig. 4) ---------------------------------------------
 namespace {
 // splits a line into numeric tokens; returns false if a token is not a number (a title line)

@@ -64,6 +64,18 @@ constexpr uint32_t kDevPosMask = 0x1FFFu, kDevNoSlot = 0x7FFFu;
 constexpr int kDevKShift = 13, kDevSlotShift = 16;
 void pack_device_edges(const TileTables &X, std::vector<double> &out);
 
+// Tables of the edge-centric two-pass kernels (SWE_KERNEL_EDGE_TWO_PASS): every edge of the mesh once,
+// in the order in which the internal cell numbering meets it.  a, b = INTERNAL cell ids of the end
+// points (a = the end point with the smaller caller id, like in the tile tables; on a boundary edge
+// b = -(tag + 128 * boundary edge number) with the same edge numbering); (lx, ly) = edge length times
+// a's unit outward normal.  cedge[3 p + k] = 2 * edge + side (side 1: cell p is end point b) for local
+// edge k of internal cell p.
+struct GlobalEdges {
+    std::vector<HostEdge> edges;
+    std::vector<int32_t> cedge;
+};
+int build_global_edges(const HostTables &T, GlobalEdges &E, std::string &err);
+
 // Reader for the paper's mesh-file layout (Fig. 4): a node table (a title line, the
 // node count on its own line, rows "id x y z") and a connectivity table (title, cell count, rows
 // "id n1 n2 n3 manning"), ids 1-based; anything after the connectivity rows (the "Ghost cells to be

@@ -59,6 +59,8 @@ constexpr uint32_t kPosMask = 0x1FFFu;
 constexpr int kKShift = 13, kSlotShift = 16;
 constexpr uint32_t kNoSlot = 0x7FFFu;
 
+struct __align__(8) GEdge { int32_t a, b; double lx, ly; };     // 24 bytes (= HostEdge, mesh_builder.h)
+
 struct Ctrl {                 // device-resident loop state
     double t[2];              // simulated time of the state in U0 / U1 (ping-pong like the state: every
                               // block reads t[cur] while block 0 writes t[cur ^ 1])
@@ -83,6 +85,11 @@ struct Params {
     int32_t *hint;            // [ntiles] 1 if the tile was active (not all dry) at the previous step
     double *pmax0, *pmax1;    // [npart] per-block max rate of state U0 / U1
     Ctrl *ctrl;
+    // edge-centric two-pass kernels only (SWE_KERNEL_EDGE_TWO_PASS; NULL otherwise)
+    const GEdge *gedges;      // [nge] every edge of the mesh once: internal cell ids of a and b, (lx, ly)
+    const int32_t *cedge;     // [nt][3] 2 * edge + side for local edge k of internal cell p
+    double *eres;             // [nge][2][3] pass-1 results: side a (o0,o1,o2), side b (-o0,-o3,-o4)
+    int32_t nge;
     int32_t nt, ntiles, npart, max_edges, max_halo;
     int32_t hll;              // 1: plain HLL for the tangential momentum too (SWE_RIEMANN_HLL)
     double g, hg, inv_g, cfl, hdry;   // hg = g/2
@@ -315,6 +322,57 @@ __device__ __forceinline__ void hllc_flux(const double g, const double hg, const
         const double G2s = (fma(SR, qL * tL, -(SL * (qR * tR))) + SS * (hR * tR - hL * tL)) * inv;
         G2 = supL ? qL * tL : (supR ? qR * tR : G2s);
     }
+}
+
+// ---- one edge: a2-a7 of SURVEY.md section 8(a) -------------------------------------------------
+// (lx, ly) = edge length times the unit outward normal n of end point a.  bword >= 0: interior edge
+// with end points A and B; bword < 0: boundary edge of A, -bword = tag + 128 * boundary edge number.
+// o[0] = L G0, (o[1], o[2]) = L (F - sb_a n), (o[3], o[4]) = L (F - sb_b n) with F = T^-1 G~ in the
+// frame of n.  Side a subtracts (o0,o1,o2)/|Omega_a|, side b adds (o0,o3,o4)/|Omega_b| (its outward
+// normal is -n).  Shared by the tiled step kernel and the edge-centric two-pass kernels.
+__device__ __forceinline__ void edge_eval(const Params &P, const double lx, const double ly, const Rec &A,
+                                          const Rec &B, const int32_t bword, const double dt, double o[5])
+{
+    const double g = P.g, hg = P.hg, hdry = P.hdry;
+    const double L2 = fma(lx, lx, ly * ly);
+    double rl;
+    const double L = fast_sqrt_rsqrt(L2, rl);
+    const double n1 = lx * rl, n2 = ly * rl;                                  // unit outward normal of a
+    const double uL = fma(A.u, n1, A.v * n2), vL = fma(A.v, n1, -(A.u * n2));   // eq.(12)
+    double G0, G1, G2, sba = 0.0, sbb = 0.0;
+    if (bword >= 0) {
+        // a2: hydrostatic reconstruction, eq.(28), R-14
+        const double zf = dmax(A.z, B.z);
+        const double hL = dmax(0.0, A.h + (A.z - zf));
+        const double hR = dmax(0.0, B.h + (B.z - zf));
+        const double uR = fma(B.u, n1, B.v * n2), vR = fma(B.v, n1, -(B.u * n2));
+        const double hL2 = hL * hL, hR2 = hR * hR;
+        hllc_flux(g, hg, P.inv_g, hdry, hL, uL, vL, hR, uR, vR, hg * hL2, hg * hR2, P.hll != 0, G0, G1, G2);
+        // bathymetry source eq.(30) with g/2 (R-13), one value per side
+        sba = hg * fma(-A.h, A.h, hL2);
+        sbb = hg * fma(-B.h, B.h, hR2);
+    } else {                                    // a6: boundary edge
+        const int bw = -bword, tag = bw & 127;
+        const double hL = A.h;
+        const double pr = hg * hL * hL;
+        if (tag == SWE_BC_WALL) { G0 = 0.0; G1 = pr; G2 = 0.0; }                 // R-4
+        else if (tag == SWE_BC_TRANSMISSIVE) {                                    // R-21
+            if (hL > hdry) { G0 = hL * uL; G1 = fma(G0, uL, pr); G2 = G0 * vL; }
+            else { G0 = 0.0; G1 = 0.0; G2 = 0.0; }
+        } else {                                                                  // R-20
+            const double qn = __ldg(P.qn_tag + tag);
+            G0 = qn; G2 = 0.0;
+            G1 = hL > hdry ? fma(qn * qn, fast_rcp(hL), pr) : 0.0;
+        }
+        // boundary diagnostics: volume that left through this edge so far.  One
+        // writer per edge, so the sum is deterministic; walls carry no mass.
+        if (tag != SWE_BC_WALL) P.bvol[bw >> 7] += G0 * L * dt;
+    }
+    // a7: rotate back (T^-1) and scale by the edge length: L (G1 n - G2 t) = G1 l - G2 l_perp
+    const double LFx = fma(G1, lx, -(G2 * ly)), LFy = fma(G1, ly, G2 * lx);
+    o[0] = L * G0;
+    o[1] = fma(-sba, lx, LFx); o[2] = fma(-sba, ly, LFy);
+    o[3] = fma(-sbb, lx, LFx); o[4] = fma(-sbb, ly, LFy);
 }
 
 // ---- one cell: a7-a10, eq.(37), PAPER.md:250 ---------------------------------------------------
@@ -583,62 +641,24 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
             const unsigned char *const se = sedge0 + s * estride;
             const uint2 *const sab = reinterpret_cast<const uint2 *>(se);
             const double2 *const slxy = reinterpret_cast<const double2 *>(se + ((ne + 1) & ~1) * 8);
-            const double g = P.g, hg = P.hg;
             for (int e = tid; e < ne; e += TC) {
                 const uint2 ab = sab[e];
                 const double2 l = slxy[e];
-                const double lx = l.x, ly = l.y;
                 const Rec A = srec[ab.x & kPosMask];
-                const double L2 = fma(lx, lx, ly * ly);
-                double rl;
-                const double L = fast_sqrt_rsqrt(L2, rl);
-                const double n1 = lx * rl, n2 = ly * rl;                                  // unit outward normal of a
-                const double uL = fma(A.u, n1, A.v * n2), vL = fma(A.v, n1, -(A.u * n2));   // eq.(12)
-                double G0, G1, G2, sba = 0.0, sbb = 0.0;
-                const bool interior = (int32_t)ab.y >= 0;
-                if (interior) {
-                    const Rec B = srec[ab.y & kPosMask];
-                    // a2: hydrostatic reconstruction, eq.(28), R-14
-                    const double zf = dmax(A.z, B.z);
-                    const double hL = dmax(0.0, A.h + (A.z - zf));
-                    const double hR = dmax(0.0, B.h + (B.z - zf));
-                    const double uR = fma(B.u, n1, B.v * n2), vR = fma(B.v, n1, -(B.u * n2));
-                    const double hL2 = hL * hL, hR2 = hR * hR;
-                    hllc_flux(g, hg, P.inv_g, hdry, hL, uL, vL, hR, uR, vR, hg * hL2, hg * hR2, P.hll != 0, G0, G1, G2);
-                    // bathymetry source eq.(30) with g/2 (R-13), one value per side
-                    sba = hg * fma(-A.h, A.h, hL2);
-                    sbb = hg * fma(-B.h, B.h, hR2);
-                } else {                                    // a6: boundary edge
-                    const int bw = -(int32_t)ab.y, tag = bw & 127;
-                    const double hL = A.h;
-                    const double pr = hg * hL * hL;
-                    if (tag == SWE_BC_WALL) { G0 = 0.0; G1 = pr; G2 = 0.0; }                 // R-4
-                    else if (tag == SWE_BC_TRANSMISSIVE) {                                    // R-21
-                        if (hL > hdry) { G0 = hL * uL; G1 = fma(G0, uL, pr); G2 = G0 * vL; }
-                        else { G0 = 0.0; G1 = 0.0; G2 = 0.0; }
-                    } else {                                                                  // R-20
-                        const double qn = __ldg(P.qn_tag + tag);
-                        G0 = qn; G2 = 0.0;
-                        G1 = hL > hdry ? fma(qn * qn, fast_rcp(hL), pr) : 0.0;
-                    }
-                    // boundary diagnostics: volume that left through this edge so far.  One
-                    // writer per edge, so the sum is deterministic; walls carry no mass.
-                    if (tag != SWE_BC_WALL) P.bvol[bw >> 7] += G0 * L * dt;
-                }
-                // a7: rotate back (T^-1) and scale by the edge length: L (G1 n - G2 t) = G1 l - G2 l_perp;
-                // side a subtracts (o0, LF - sb_a l) / |Omega_a|, side b adds (o0, LF - sb_b l) / |Omega_b|
-                // (its outward normal is -n): b's slot gets the negated values
-                const double LFx = fma(G1, lx, -(G2 * ly)), LFy = fma(G1, ly, G2 * lx);
-                const double o0 = L * G0;
+                Rec B = A;
+                if ((int32_t)ab.y >= 0) B = srec[ab.y & kPosMask];
+                double o[5];
+                edge_eval(P, l.x, l.y, A, B, (int32_t)ab.y, dt, o);
+                // b's slot gets the negated values (its outward normal is -n)
                 const unsigned sa = ab.x >> kSlotShift;
                 if (sa != kNoSlot) {
-                    so01[sa] = make_double2(o0, fma(-sba, lx, LFx));
-                    so2[sa] = fma(-sba, ly, LFy);
+                    so01[sa] = make_double2(o[0], o[1]);
+                    so2[sa] = o[2];
                 }
                 const unsigned sb = ab.y >> kSlotShift;      // boundary words have bit 31 set: > kNoSlot
                 if (sb < kNoSlot) {
-                    so01[sb] = make_double2(-o0, fma(sbb, lx, -LFx));
-                    so2[sb] = fma(sbb, ly, -LFy);
+                    so01[sb] = make_double2(-o[0], -o[3]);
+                    so2[sb] = -o[4];
                 }
             }
             __syncthreads();

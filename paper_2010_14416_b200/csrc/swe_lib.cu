@@ -79,6 +79,82 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
     }
 }
 
+// ---- edge-centric two-pass alternative (SWE_KERNEL_EDGE_TWO_PASS) -------------
+// The time step of a launch: dt = CFL / max of the per-block maxima, clipped to t_end (swe_run_until).
+__device__ __forceinline__ double launch_dt(const Params &P, const int cur, double *s_red, double &dt_cfl,
+                                            double &t_now, bool &clipped)
+{
+    dt_cfl = reduce_dt(P, P.pmax(cur), s_red);
+    t_now = __ldcg(&P.ctrl->t[cur]);
+    const double left = __ldcg(&P.ctrl->t_end) - t_now;
+    clipped = dt_cfl >= left;
+    return fmax(clipped ? left : dt_cfl, 0.0);
+}
+
+// pass 1: one thread per edge of the mesh (a2-a7): both end points' records are gathered from HBM / L2
+// (one 32-byte sector each), the result for each side is written once
+__global__ void __launch_bounds__(256)
+swe_edge_pass_kernel(const Params P, const int cur)
+{
+    __shared__ double s_red[32];
+    double dt_cfl, t_now; bool clipped;
+    const double dt = launch_dt(P, cur, s_red, dt_cfl, t_now, clipped);
+    const Rec *__restrict__ U = P.U(cur);
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < P.nge; e += (long long)gridDim.x * blockDim.x) {
+        const int2 ab = __ldg(reinterpret_cast<const int2 *>(P.gedges + e));
+        const double2 l = make_double2(__ldg(&P.gedges[e].lx), __ldg(&P.gedges[e].ly));   // 24-byte records: 8-byte aligned
+        const Rec A = load_rec(U + ab.x);
+        Rec B = A;
+        if (ab.y >= 0) B = load_rec(U + ab.y);
+        double o[5];
+        edge_eval(P, l.x, l.y, A, B, ab.y, dt, o);
+        double2 *r = reinterpret_cast<double2 *>(P.eres + 6 * e);
+        r[0] = make_double2(o[0], o[1]);
+        r[1] = make_double2(o[2], -o[0]);
+        r[2] = make_double2(-o[3], -o[4]);
+    }
+}
+
+// pass 2: one thread per cell (a7-a11): its three edge results in the order k = 0,1,2, friction,
+// update, local rate; per-block maximum; block 0 advances the device clock
+__global__ void __launch_bounds__(256)
+swe_cell_pass_kernel(const Params P, const int cur, const int tile_cells)
+{
+    __shared__ double s_red[32];
+    double dt_cfl, t_now; bool clipped;
+    const double dt = launch_dt(P, cur, s_red, dt_cfl, t_now, clipped);
+    const Rec *__restrict__ Uin = P.U(cur);
+    Rec *__restrict__ Uout = P.U(cur ^ 1);
+    double rate = 0.0;
+    unsigned nclamp = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P.nt; i += (long long)gridDim.x * blockDim.x) {
+        const int32_t c0 = __ldg(P.cedge + 3 * i), c1 = __ldg(P.cedge + 3 * i + 1), c2 = __ldg(P.cedge + 3 * i + 2);
+        const double *r0 = P.eres + 3 * (size_t)c0, *r1 = P.eres + 3 * (size_t)c1, *r2 = P.eres + 3 * (size_t)c2;
+        // three edges in the fixed order k = 0,1,2 (R-17)
+        const double s1 = (__ldcg(r0) + __ldcg(r1)) + __ldcg(r2);
+        const double s2 = (__ldcg(r0 + 1) + __ldcg(r1 + 1)) + __ldcg(r2 + 1);
+        const double s3 = (__ldcg(r0 + 2) + __ldcg(r1 + 2)) + __ldcg(r2 + 2);
+        const Rec Ui = load_rec(Uin + i);
+        const int t = (int)(i / tile_cells), q = (int)(i - (long long)t * tile_cells);
+        const double *cc = P.cellc + (size_t)t * 3 * tile_cells + q;
+        Rec Un;
+        rate = fmax(rate, cell_update(P, Ui, s1, s2, s3, __ldg(cc), __ldg(cc + tile_cells), __ldg(cc + 2 * tile_cells), dt, Un, nclamp));
+        store_rec(Uout + i, Un);
+    }
+    rate = block_max(rate, s_red);
+    if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
+    if (threadIdx.x == 0) {
+        P.pmax(cur ^ 1)[blockIdx.x] = rate;
+        if (blockIdx.x == 0) {
+            Ctrl *c = P.ctrl;
+            c->t[cur ^ 1] = clipped ? fmax(__ldcg(&P.ctrl->t_end), t_now) : t_now + dt;    // R-24
+            if (dt > 0.0) { c->dt_last = dt; c->steps += 1; }
+            if (!(dt_cfl > 0.0)) c->all_dry = 1;
+            c->n_active += (unsigned long long)P.ntiles;      // no dry-tile shortcut on this path
+        }
+    }
+}
+
 typedef void (*step_kernel_t)(const Params, int, const long long);
 step_kernel_t step_kernel_for(int tc)
 {
@@ -186,6 +262,8 @@ struct swe_mesh {
     swe_params prm;
     HostTables T;
     TileTables X;
+    GlobalEdges E;            // SWE_KERNEL_EDGE_TWO_PASS only
+    bool edge_kernel = false; int grid_edge = 0, grid_cell = 0;
     std::string err;
     // device
     bool bound = false, have_state = false, have_rates = false;
@@ -222,9 +300,9 @@ namespace {
 static_assert(sizeof(HostEdge) == 24 && kDevPosMask == kPosMask && kDevKShift == kKShift && kDevSlotShift == kSlotShift &&
               kDevNoSlot == kNoSlot, "edge list encoding (mesh_builder.h / swe_kernels.cuh)");
 struct Layout {
-    size_t U0, U1, cellc, edges, tinfo, bvol, hint, zcell, perm, stage, pmax0, pmax1, qn, ctrl, total;
+    size_t U0, U1, cellc, edges, tinfo, bvol, hint, zcell, perm, stage, pmax0, pmax1, qn, ctrl, gedges, cedge, eres, total;
 };
-Layout make_layout(const HostTables &T, const TileTables &X)
+Layout make_layout(const HostTables &T, const TileTables &X, const GlobalEdges &E)
 {
     Layout L; size_t o = 0; const size_t n = (size_t)T.nt;
     auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
@@ -237,6 +315,8 @@ Layout make_layout(const HostTables &T, const TileTables &X)
     L.stage = take(3 * n * sizeof(double));
     L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
     L.qn = take((SWE_BC_MAX_TAG + 1) * sizeof(double)); L.ctrl = take(sizeof(Ctrl));
+    L.gedges = take(E.edges.size() * sizeof(HostEdge)); L.cedge = take(E.cedge.size() * sizeof(int32_t));
+    L.eres = take(E.edges.size() * 6 * sizeof(double));
     L.total = o;
     return L;
 }
@@ -249,6 +329,7 @@ int swe_params_default(swe_params *p)
     if (!p) return SWE_ERR_INVALID_ARG;
     p->g = 9.81; p->cfl = 0.9; p->h_dry = 1e-6;
     p->ordering = SWE_ORDER_HILBERT; p->block_size = 0; p->loop_mode = SWE_LOOP_AUTO; p->riemann = SWE_RIEMANN_HLLC;
+    p->kernel = SWE_KERNEL_TILED; p->reserved = 0;
     return SWE_OK;
 }
 
@@ -269,6 +350,7 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     if (params) p = *params;
     if (!(p.g > 0.0) || !(p.cfl > 0.0) || !(p.h_dry >= 0.0) || p.ordering < 0 || p.ordering > SWE_ORDER_RCM ||
         p.loop_mode < 0 || p.loop_mode > SWE_LOOP_LAUNCH || p.riemann < 0 || p.riemann > SWE_RIEMANN_HLL ||
+        p.kernel < 0 || p.kernel > SWE_KERNEL_EDGE_TWO_PASS ||
         (p.block_size != 0 && p.block_size != 64 && p.block_size != 128 && p.block_size != 192 && p.block_size != 256)) {
         g_create_err = "swe_mesh_create: invalid swe_params (block_size must be 0, 64, 128, 192 or 256)";
         return SWE_ERR_INVALID_ARG;
@@ -284,6 +366,11 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     m->block = p.block_size ? p.block_size : kDefaultBlock;
     rc = build_tiles(m->T, m->block, p.g, m->X, m->err);
     if (rc != SWE_OK) { g_create_err = m->err; delete m; return rc; }
+    m->edge_kernel = p.kernel == SWE_KERNEL_EDGE_TWO_PASS;
+    if (m->edge_kernel) {
+        rc = build_global_edges(m->T, m->E, m->err);
+        if (rc != SWE_OK) { g_create_err = m->err; delete m; return rc; }
+    }
     *out = m;
     return SWE_OK;
 }
@@ -315,7 +402,7 @@ int swe_mesh_destroy(swe_mesh *m)
 int swe_mesh_workspace_bytes(const swe_mesh *m, size_t *bytes)
 {
     if (!m || !bytes) return SWE_ERR_INVALID_ARG;
-    *bytes = make_layout(m->T, m->X).total;
+    *bytes = make_layout(m->T, m->X, m->E).total;
     return SWE_OK;
 }
 
@@ -358,6 +445,13 @@ int swe_get_step_bytes(const swe_mesh *m, double active_tiles, double edge_lists
     if (!m || !bytes || !(active_tiles >= 0.0) || !(edge_lists >= 0.0)) return SWE_ERR_INVALID_ARG;
     const TileTables &X = m->X;
     const double nt = (double)m->T.nt, ntiles = (double)X.ntiles, TC = (double)X.tile_cells;
+    if (m->edge_kernel) {
+        // pass 1: edge record, one sector per end point, both sides' results out; pass 2: edge ids,
+        // three 24-byte results, record in and out, cell constants
+        const double ne = (double)m->E.edges.size(), nb = (double)X.nbedges;
+        *bytes = ne * 24.0 + (2.0 * ne - nb) * 32.0 + ne * 48.0 + nt * (12.0 + 72.0 + 32.0 + 24.0 + 32.0);
+        return SWE_OK;
+    }
     double b = 0.0;
     b += 32.0 * nt;                                   // every cell's record read (TMA bulk copy) ...
     b += 32.0 * nt;                                   // ... and written (256-bit store)
@@ -410,7 +504,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     if (!m || !device_workspace) return SWE_ERR_INVALID_ARG;
     const HostTables &T = m->T;
     const size_t n = (size_t)T.nt;
-    const Layout L = make_layout(T, m->X);
+    const Layout L = make_layout(T, m->X, m->E);
     if (bytes < L.total || ((uintptr_t)device_workspace & 255u)) {
         m->err = "workspace too small or not 256-byte aligned";
         return SWE_ERR_WORKSPACE;
@@ -450,6 +544,14 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     // blocks own two tiles (12.8 vs 14.9 us at 200 000 cells), so AUTO means GRAPH
     if (mode == SWE_LOOP_AUTO) mode = SWE_LOOP_GRAPH;
     if (mode == SWE_LOOP_PERSISTENT && !coop) mode = SWE_LOOP_GRAPH;
+    if (m->edge_kernel) {
+        // two kernels per step: the kernel boundary is the only grid-wide barrier they have
+        if (mode == SWE_LOOP_PERSISTENT) mode = SWE_LOOP_GRAPH;
+        const int64_t want_e = ((int64_t)m->E.edges.size() + 255) / 256, want_c = ((int64_t)n + 255) / 256;
+        m->grid_edge = (int)std::max<int64_t>(1, std::min<int64_t>(want_e, (int64_t)sms * 8));
+        m->grid_cell = (int)std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(want_c, (int64_t)sms * 8), kMaxPart));
+        m->grid = m->coop_grid = m->grid_cell;     // the per-block maxima are pass 2's
+    }
     m->loop_mode = mode;
 
     Params &P = m->P;
@@ -464,6 +566,10 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     m->d_qn = (double *)(m->ws + L.qn); P.qn_tag = m->d_qn;
     P.ctrl = (Ctrl *)(m->ws + L.ctrl);
     P.hll = m->prm.riemann == SWE_RIEMANN_HLL;
+    P.gedges = m->edge_kernel ? (const GEdge *)(m->ws + L.gedges) : nullptr;
+    P.cedge = m->edge_kernel ? (const int32_t *)(m->ws + L.cedge) : nullptr;
+    P.eres = m->edge_kernel ? (double *)(m->ws + L.eres) : nullptr;
+    P.nge = (int32_t)m->E.edges.size();
     P.nt = (int32_t)T.nt; P.ntiles = ntiles; P.max_edges = X.max_edges; P.max_halo = X.max_halo;
     P.npart = mode == SWE_LOOP_PERSISTENT ? m->coop_grid : m->grid;
     P.g = m->prm.g; P.hg = 0.5 * m->prm.g; P.inv_g = 1.0 / m->prm.g; P.cfl = m->prm.cfl;
@@ -478,6 +584,10 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
         pack_device_edges(X, dev_edges);
         CK(cudaMemcpyAsync(m->ws + L.edges, dev_edges.data(), dev_edges.size() * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.tinfo, X.tinfo.data(), X.tinfo.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        if (m->edge_kernel) {
+            CK(cudaMemcpyAsync(m->ws + L.gedges, m->E.edges.data(), m->E.edges.size() * sizeof(HostEdge), cudaMemcpyHostToDevice, s));
+            CK(cudaMemcpyAsync(m->ws + L.cedge, m->E.cedge.data(), m->E.cedge.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        }
         CK(cudaMemcpyAsync(m->d_zcell, T.cell_z.data(), n * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_inv, T.inv.data(), n * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->d_qn, m->qn_tag, sizeof(m->qn_tag), cudaMemcpyHostToDevice, s));
@@ -591,12 +701,24 @@ int swe_compute_dt(swe_mesh *m, double *dt_out)
     return SWE_OK;
 }
 
+// one time step on stream st from the state in buffer cur: the fused tile kernel, or the two passes
+static void launch_step(swe_mesh *m, cudaStream_t st, int cur)
+{
+    if (m->edge_kernel) {
+        swe_edge_pass_kernel<<<m->grid_edge, 256, 0, st>>>(m->P, cur);
+        swe_cell_pass_kernel<<<m->grid_cell, 256, 0, st>>>(m->P, cur, m->X.tile_cells);
+    } else {
+        m->kern<<<m->grid, m->block, m->smem, st>>>(m->P, cur, 1);
+    }
+}
+static int kernels_per_step(const swe_mesh *m) { return m->edge_kernel ? 2 : 1; }
+
 static int launch_steps_direct(swe_mesh *m, int64_t n)
 {
     for (int64_t s = 0; s < n; s++) {
-        m->kern<<<m->grid, m->block, m->smem, m->stream>>>(m->P, m->cur, 1);
+        launch_step(m, m->stream, m->cur);
         m->cur ^= 1;
-        m->launches++;
+        m->launches += kernels_per_step(m);
     }
     CK(cudaGetLastError());
     return SWE_OK;
@@ -614,7 +736,7 @@ static int graph_for(swe_mesh *m, int steps, cudaGraphExec_t *out)
     cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
     int c = m->cur;
     if (e == cudaSuccess) {
-        for (int s = 0; s < steps; s++) { m->kern<<<m->grid, m->block, m->smem, cap>>>(m->P, c, 1); c ^= 1; }
+        for (int s = 0; s < steps; s++) { launch_step(m, cap, c); c ^= 1; }
         e = cudaStreamEndCapture(cap, &g);
     }
     if (e == cudaSuccess) e = cudaGraphInstantiate(&ex, g, 0);
@@ -652,7 +774,7 @@ int swe_run(swe_mesh *m, int64_t nsteps)
             rc = graph_for(m, chunks[q], &ex);
             if (rc != SWE_OK) return rc;
             CK(cudaGraphLaunch(ex, m->stream));
-            m->launches += chunks[q];
+            m->launches += (int64_t)chunks[q] * kernels_per_step(m);
             left -= chunks[q];
         }
     }

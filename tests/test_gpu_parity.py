@@ -254,6 +254,44 @@ def test_config5_sweep_2M_both_orderings(ordering):
     assert_parity(m, o, w)
 
 
+# ---- NEXT-2: the edge-centric two-pass kernels (PAPER.md:393, :617 leave the kernel split open) ----
+@pytest.mark.parametrize("loop_mode", [B.LOOP_GRAPH, B.LOOP_LAUNCH])
+def test_edge_two_pass_kernel_matches_oracle_and_tiled_kernel(loop_mode):
+    """Pass 1 (one thread per edge of the mesh) + pass 2 (one thread per cell): the same scheme as
+    the fused tile kernel, against the oracle at the same bar, river case with inflow / outflow /
+    wet-dry fronts / friction; and against the tile kernel itself (same edge and cell arithmetic,
+    same order k = 0,1,2; the compiler contracts the two instantiations differently, so they agree
+    to round-off, not to the bit)."""
+    w = W.config4(nx=320, ny=80)
+    m, o = run_both(w, 600, kernel=B.KERNEL_EDGE_TWO_PASS, loop_mode=loop_mode)
+    got = assert_parity(m, o, w)
+    np.testing.assert_allclose(m.get_boundary_volumes(), o.boundary_volumes(), rtol=1e-10, atol=1e-10)
+    r = B.SweMesh.from_workload(w).bind_device()
+    r.set_state(w.h, w.hu, w.hv)
+    r.run(600)
+    ref = r.get_state()
+    for a, b in zip(got[:3], ref[:3]):
+        np.testing.assert_allclose(a, b, rtol=1e-12, atol=1e-12)
+    assert got[3] == pytest.approx(ref[3], rel=1e-14)
+
+
+def test_edge_two_pass_kernel_ordering_invariance_and_run_until():
+    w = W.config2(nx=300, ny=30)
+    out = []
+    for ordering in (B.ORDER_IDENTITY, B.ORDER_HILBERT):
+        m = B.SweMesh.from_workload(w, ordering=ordering, kernel=B.KERNEL_EDGE_TWO_PASS).bind_device()
+        m.set_state(w.h, w.hu, w.hv)
+        n = m.run_until(1.5)
+        out.append(m.get_state() + (n,))
+    for a, b in zip(out[0][:3], out[1][:3]):
+        np.testing.assert_array_equal(a, b)
+    assert out[0][3] == out[1][3] == 1.5 and out[0][5] == out[1][5]
+    o = OracleSolver.from_workload(w)
+    assert o.run_until(1.5) == out[0][5]
+    for a, b in zip(out[0][:3], o.get_state()[:3]):
+        np.testing.assert_allclose(a, b, rtol=RTOL, atol=ATOL)
+
+
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times (defaults) ----------
 def test_config3_full_size_every_cell_then_invariants():
     """configs[2] at 2000x1000 squares (4,000,000 cells): every cell against the oracle after 40

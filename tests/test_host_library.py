@@ -25,7 +25,7 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_struct_sizes_match_header():
-    assert ctypes.sizeof(B.SweParams) == 3 * 8 + 4 * 4
+    assert ctypes.sizeof(B.SweParams) == 3 * 8 + 6 * 4
     assert ctypes.sizeof(B.SweStats) == 3 * 8 + 6 * 8
     p = B.SweParams()
     B.load_library().swe_params_default(ctypes.byref(p))
