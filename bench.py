@@ -270,7 +270,7 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     n = w.ncells
     order = {"hilbert": B.ORDER_HILBERT, "rcm": B.ORDER_RCM, "identity": B.ORDER_IDENTITY}[args.ordering]
     loop = {"auto": B.LOOP_AUTO, "graph": B.LOOP_GRAPH, "persistent": B.LOOP_PERSISTENT,
-            "launch": B.LOOP_LAUNCH}[args.loop]
+            "launch": B.LOOP_LAUNCH, "cluster": B.LOOP_CLUSTER}[args.loop]
     # ---- device-resident leg of the headline workload -------------------------------------
     r = measure_device(B, w, args, dev, order, loop, barrier, world, ClockSampler(local_rank))
     m, ms, info, tiles, stats = r["mesh"], r["ms"], r["info"], r["tiles"], r["stats"]
@@ -367,7 +367,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--workload", default="config4")
     ap.add_argument("--ordering", default="hilbert", choices=["hilbert", "rcm", "identity"])
-    ap.add_argument("--loop", default="auto", choices=["auto", "graph", "persistent", "launch"])
+    ap.add_argument("--loop", default="auto", choices=["auto", "graph", "persistent", "launch", "cluster"])
     ap.add_argument("--block", type=int, default=0, help="cells per tile = threads per block (0 = default)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-wet", dest="wet", action="store_false",

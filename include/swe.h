@@ -71,8 +71,13 @@ enum { SWE_RIEMANN_HLLC = 0, SWE_RIEMANN_HLL = 1 };
 enum { SWE_KERNEL_TILED = 0, SWE_KERNEL_EDGE_TWO_PASS = 1 };
 /* swe_params.loop_mode: how swe_run iterates without host round trips: GRAPH = CUDA graphs of
  * 128 / 16 / 2 step-kernel launches, PERSISTENT = one cooperative launch with a grid barrier per
- * step, LAUNCH = plain launches; AUTO = GRAPH (measured as fast or faster at every mesh size) */
-enum { SWE_LOOP_AUTO = 0, SWE_LOOP_GRAPH = 1, SWE_LOOP_PERSISTENT = 2, SWE_LOOP_LAUNCH = 3 };
+ * step, LAUNCH = plain launches, CLUSTER = meshes of at most 16 tiles only: one launch of one
+ * thread-block cluster, one CTA per tile, state resident in shared memory for the whole run, halo
+ * records through distributed shared memory, the hardware cluster barrier per step (PAPER.md:517:
+ * small meshes are "strictly limited by latencies").  AUTO = CLUSTER when the mesh fits (with
+ * block_size 0: tiles of 128 cells, up to 2048 cells), else GRAPH (as fast as or faster than
+ * PERSISTENT at every larger mesh size).  All modes give bit-identical results. */
+enum { SWE_LOOP_AUTO = 0, SWE_LOOP_GRAPH = 1, SWE_LOOP_PERSISTENT = 2, SWE_LOOP_LAUNCH = 3, SWE_LOOP_CLUSTER = 4 };
 
 typedef struct {
     double g;           /* gravitational acceleration; the paper gives no value, default 9.81 */
@@ -80,7 +85,8 @@ typedef struct {
     double h_dry;       /* wet/dry threshold: a cell or edge side is dry iff h <= h_dry; 1e-6.
                            Values below 1e-250 act as 1e-250 (keeps every rsqrt argument normal) */
     int32_t ordering;   /* SWE_ORDER_*; default SWE_ORDER_HILBERT */
-    int32_t block_size; /* cells per tile = CUDA threads per block: 64, 128, 192 or 256; 0 = default (192) */
+    int32_t block_size; /* cells per tile (= CUDA threads per block, twice that in CLUSTER mode): 64, 128, 192 or
+                           256; 0 = default (192; 128 for meshes that AUTO runs in CLUSTER mode) */
     int32_t loop_mode;  /* SWE_LOOP_*; default SWE_LOOP_AUTO */
     int32_t riemann;    /* SWE_RIEMANN_*; default SWE_RIEMANN_HLLC */
     int32_t kernel;     /* SWE_KERNEL_*; default SWE_KERNEL_TILED */

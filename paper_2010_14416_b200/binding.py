@@ -16,10 +16,10 @@ from . import build as _build
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
 ORDER_IDENTITY, ORDER_HILBERT, ORDER_RCM = 0, 1, 2
-LOOP_AUTO, LOOP_GRAPH, LOOP_PERSISTENT, LOOP_LAUNCH = 0, 1, 2, 3
+LOOP_AUTO, LOOP_GRAPH, LOOP_PERSISTENT, LOOP_LAUNCH, LOOP_CLUSTER = 0, 1, 2, 3, 4
 RIEMANN_HLLC, RIEMANN_HLL = 0, 1
 KERNEL_TILED, KERNEL_EDGE_TWO_PASS = 0, 1
-LOOP_NAMES = {0: "auto", 1: "graph", 2: "persistent", 3: "launch"}
+LOOP_NAMES = {0: "auto", 1: "graph", 2: "persistent", 3: "launch", 4: "cluster"}
 ERR_ALL_DRY = -9
 
 # every symbol include/swe.h declares

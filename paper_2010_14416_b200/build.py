@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libswe_b200.so")
 SOURCES = ["swe_lib.cu", "mesh_builder.cpp"]
 HEADERS = ["swe_kernels.cuh", "mesh_builder.h", os.path.join("..", "..", "include", "swe.h")]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "--fmad=false", "-lineinfo", "-std=c++17",
               "--cudart", "static", "-Xcompiler", "-fPIC,-O2,-Wall", "-shared"]
 
 

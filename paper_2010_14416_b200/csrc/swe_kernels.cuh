@@ -34,7 +34,10 @@
 // argument is a normal positive number by construction) instead of the IEEE-rounded division /
 // square-root sequences, compare-and-select instead of fmax/fmin (no NaN can reach them), end
 // point words that hold ready-made shared-memory indices, vector shared-memory accesses.
-// DESIGN.md section 7 derives why this stays inside the 1e-10 parity bar.
+// DESIGN.md section 7 derives why this stays inside the 1e-10 parity bar.  The library is compiled
+// with --fmad=false and every fused multiply-add is written out as fma(): the arithmetic is then
+// fixed by the source, so the tile kernel, the cluster loop and the edge-centric kernels, which all
+// instantiate edge_eval / cell_update, produce identical bits.
 #pragma once
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
@@ -293,11 +296,11 @@ __device__ __forceinline__ void hllc_flux(const double g, const double hg, const
         dh = hR - hL;
     } else if (wR) {                                        // eq.(26) line 1: left side dry
         const double aR = fast_sqrt(g * hR);
-        SL = uR - 2.0 * aR; SR = uR + aR;
+        SL = fma(-2.0, aR, uR); SR = uR + aR;
         qL = 0.0; GL1 = 0.0; qR = hR * uR; GR1 = fma(qR, uR, pR); dh = hR;
     } else if (wL) {                                        // eq.(26) line 2 (R-18): right side dry
         const double aL = fast_sqrt(g * hL);
-        SL = uL - aL; SR = uL + 2.0 * aL;
+        SL = uL - aL; SR = fma(2.0, aL, uL);
         qR = 0.0; GR1 = 0.0; qL = hL * uL; GL1 = fma(qL, uL, pL); dh = -hL;
     } else {
         G0 = 0.0; G1 = 0.0; G2 = 0.0;
@@ -308,7 +311,7 @@ __device__ __forceinline__ void hllc_flux(const double g, const double hg, const
     // eq.(18) in the star region; eq.(17), R-11: S_L >= 0 first, then S_R <= 0 (selected below)
     const double inv = fast_rcp(SR - SL);
     const double SS = SR * SL;
-    const double G0s = (fma(SR, qL, -(SL * qR)) + SS * dh) * inv;
+    const double G0s = fma(SS, dh, fma(SR, qL, -(SL * qR))) * inv;
     const double G1s = fma(SL * inv, fma(SR, qR - qL, -(GR1 - GL1)), GL1);      // R-12
     const bool supL = SL >= 0.0, supR = SR <= 0.0;
     G0 = supL ? qL : (supR ? qR : G0s);
@@ -319,7 +322,7 @@ __device__ __forceinline__ void hllc_flux(const double g, const double hg, const
     // in the supercritical cases G0 = qL > 0 / qR < 0 picks the upwind side as eq.(17) does.
     G2 = G0 * (G0 >= 0.0 ? tL : tR);
     if (hll) {       // plain HLL: eq.(18) for the third component too
-        const double G2s = (fma(SR, qL * tL, -(SL * (qR * tR))) + SS * (hR * tR - hL * tL)) * inv;
+        const double G2s = fma(SS, fma(hR, tR, -(hL * tL)), fma(SR, qL * tL, -(SL * (qR * tR)))) * inv;
         G2 = supL ? qL * tL : (supR ? qR * tR : G2s);
     }
 }
@@ -366,7 +369,7 @@ __device__ __forceinline__ void edge_eval(const Params &P, const double lx, cons
         }
         // boundary diagnostics: volume that left through this edge so far.  One
         // writer per edge, so the sum is deterministic; walls carry no mass.
-        if (tag != SWE_BC_WALL) P.bvol[bw >> 7] += G0 * L * dt;
+        if (tag != SWE_BC_WALL) P.bvol[bw >> 7] = fma(G0 * L, dt, P.bvol[bw >> 7]);
     }
     // a7: rotate back (T^-1) and scale by the edge length: L (G1 n - G2 t) = G1 l - G2 l_perp
     const double LFx = fma(G1, lx, -(G2 * ly)), LFy = fma(G1, ly, G2 * lx);
@@ -496,7 +499,7 @@ template <int TC> struct SmemLayout {
     static constexpr int so2 = so01 + 3 * PLC * 16;
     static constexpr int scell = (so2 + 3 * PLC * 8 + 15) & ~15;
     static constexpr int bar = scell + 3 * TC * 8;
-    static constexpr int srec = (bar + kNumBars * 8 + 31) & ~31;
+    static constexpr int srec = (bar + kNumBars * 8 + 8 + 31) & ~31;     // + two diagnostic counters
 };
 __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int ME)
 {
@@ -504,7 +507,7 @@ __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int M
     size_t o = 3 * PLC * 16;
     o = (o + 3 * PLC * 8 + 15) & ~(size_t)15;
     o += 3 * (size_t)TC * 8;
-    o = (o + kNumBars * 8 + 31) & ~(size_t)31;
+    o = (o + kNumBars * 8 + 8 + 31) & ~(size_t)31;
     o += 2 * (size_t)(TC + MH) * sizeof(Rec);
     o += 2 * (size_t)ME * 24;
     return o;
@@ -520,8 +523,7 @@ struct PipeState { unsigned n = 0, epar = 0, cpar = 0; };
 template <int TC>
 __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *smem,
                                              const Rec *__restrict__ Uin, Rec *__restrict__ Uout,
-                                             const double dt, unsigned &nclamp, unsigned &nactive,
-                                             unsigned &nelists, PipeState &ps)
+                                             const double dt, unsigned &nclamp, PipeState &ps)
 {
     typedef SmemLayout<TC> SL;
     constexpr int PLC = SL::PLC;
@@ -529,6 +531,8 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
     double *const so2 = reinterpret_cast<double *>(smem + SL::so2);
     const double *const scell = reinterpret_cast<const double *>(smem + SL::scell);
     uint64_t *const bar = reinterpret_cast<uint64_t *>(smem + SL::bar);      // rec 0,1; edge 2,3; cell 4
+    // diagnostics kept by the producer thread: [0] active tiles, [1] edge lists fetched (this launch)
+    volatile unsigned *const scount = reinterpret_cast<volatile unsigned *>(bar + kNumBars);
     Rec *const srec0 = reinterpret_cast<Rec *>(smem + SL::srec);
     const int rstride = TC + P.max_halo;
     unsigned char *const sedge0 = reinterpret_cast<unsigned char *>(srec0 + 2 * rstride);
@@ -553,7 +557,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
         const unsigned bytes = (unsigned)((ne + 1) & ~1) * 24u;        // lists are padded to an even length
         mbar_expect_tx(bar + 2 + s, bytes);
         bulk_g2s(sedge0 + s * estride, P.edges + 3 * (size_t)e0, bytes, bar + 2 + s);
-        nelists++;
+        scount[1]++;
     };
     auto issue_cellc = [&](int t) {
         mbar_expect_tx(bar + 4, 3u * TC * 8u);
@@ -575,6 +579,8 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
         }
     };
     auto load_hdr = [&](int t) { return __ldg(reinterpret_cast<const int4 *>(P.tinfo + (size_t)t * istride)); };
+    auto hdr_ne = [](int4 h) { return h.y; };
+    auto hdr_nh = [](int4 h) { return h.z; };
     auto load_hid = [&](int t) { return tid < P.max_halo ? __ldg(P.tinfo + (size_t)t * istride + kInfoHdr + tid) : -1; };
 
     // ---- prologue: everything tile n needs; header, halo id and hint of tile n+1
@@ -583,16 +589,16 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
     bool req0 = true;                    // was this tile's edge list requested?  The step's first tile: always
     if (producer) {
         issue_recs(tile, n & 1);
-        issue_edges(hdr0.x, hdr0.y, n & 1);
+        issue_edges(hdr0.x, hdr_ne(hdr0), n & 1);
     }
     if (tile + G < P.ntiles) { hdr1 = load_hdr(tile + G); hid1 = load_hid(tile + G); hint1 = ldcg_i32(P.hint + tile + G); }
-    gather_halo(tile, hdr0.z, hid0, n & 1);
+    gather_halo(tile, hdr_nh(hdr0), hid0, n & 1);
     cp_async_commit();
     for (;;) {
         const int s = n & 1;
         const int base = tile * TC;
         const bool have_next = tile + G < P.ntiles;
-        const int ne = hdr0.y, nh = hdr0.z;
+        const int ne = hdr_ne(hdr0), nh = hdr_nh(hdr0);
         // ---- top
         cp_async_wait<0>();                               // own halo gathers of this tile
         mbar_wait(bar + s, (n >> 1) & 1u);
@@ -612,13 +618,13 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
                 // list, so the list of the NEXT tile is requested only if that tile was active at the
                 // previous step; a tile that turns out active without its list (the wet front reached
                 // it) fetches it on the spot, below.
-                if (hint1) issue_edges(hdr1.x, hdr1.y, s ^ 1);
+                if (hint1) issue_edges(hdr1.x, hdr_ne(hdr1), s ^ 1);
             }
             if (active) issue_cellc(tile);
             P.hint[tile] = active;
-            nactive += active;
+            scount[0] += active;
         }
-        if (have_next) gather_halo(tile + G, hdr1.z, hid1, s ^ 1);
+        if (have_next) gather_halo(tile + G, hdr_nh(hdr1), hid1, s ^ 1);
         cp_async_commit();
         int4 hdr2 = make_int4(0, 0, 0, 0);
         int hid2 = -1, hint2 = 0;
@@ -685,6 +691,156 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
     cp_async_wait<0>();
     ps.n = n + 1; ps.epar = epar; ps.cpar = cpar;
     return rate;
+}
+
+// ---- small meshes: the whole time loop in ONE thread-block cluster ---------------------------------
+// small meshes are "strictly limited by latencies" of kernel launches.  A mesh of at
+// most 16 tiles runs swe_run(nsteps) as one launch of one cluster, one CTA per tile: the tile's state
+// (double-buffered), edge list and cell constants stay in its shared memory for the whole run; halo
+// records are read from the owning CTA's shared memory (distributed shared memory); the per-tile
+// maximum rate is stored into every CTA's shared memory, so the next dt needs no global memory; and
+// the step boundary is the hardware cluster barrier instead of a kernel boundary or a grid barrier.
+// NT = 2 TC threads per CTA, so the ~1.66 TC edges of a tile take ONE pass of the edge loop.
+// Same edge_eval / cell_update, same edge orientation and summation order as the tile kernel: the
+// results are bit-identical to the other loop modes.
+constexpr int kMaxClusterTiles = 16;
+template <int TC> struct ClusterLayout {
+    static constexpr int PLC = TC + 1;
+    static constexpr int so01 = 0;
+    static constexpr int so2 = so01 + 3 * PLC * 16;
+    static constexpr int scell = (so2 + 3 * PLC * 8 + 15) & ~15;
+    static constexpr int smax = scell + 3 * TC * 8;
+    static constexpr int srec = (smax + 2 * kMaxClusterTiles * 8 + 31) & ~31;
+};
+__host__ __device__ __forceinline__ size_t cluster_smem_bytes(int TC, int MH, int ME)
+{
+    const size_t PLC = (size_t)TC + 1;
+    size_t o = 3 * PLC * 16;
+    o = (o + 3 * PLC * 8 + 15) & ~(size_t)15;
+    o += 3 * (size_t)TC * 8 + 2 * kMaxClusterTiles * 8;
+    o = (o + 31) & ~(size_t)31;
+    return o + 2 * (size_t)(TC + MH) * sizeof(Rec) + (size_t)ME * 24;
+}
+
+template <int TC>
+__device__ __forceinline__ void cluster_loop(const Params &P, unsigned char *smem, double *s_red, int cur,
+                                             const long long nsteps)
+{
+    namespace cg = cooperative_groups;
+    typedef ClusterLayout<TC> CL;
+    constexpr int PLC = CL::PLC, NT = 2 * TC;
+    cg::cluster_group cluster = cg::this_cluster();
+    double2 *const so01 = reinterpret_cast<double2 *>(smem + CL::so01);
+    double *const so2 = reinterpret_cast<double *>(smem + CL::so2);
+    double *const scell = reinterpret_cast<double *>(smem + CL::scell);
+    double *const smax = reinterpret_cast<double *>(smem + CL::smax);           // [2][kMaxClusterTiles]
+    Rec *const srec0 = reinterpret_cast<Rec *>(smem + CL::srec);
+    const int rstride = TC + P.max_halo;
+    unsigned char *const sedge = reinterpret_cast<unsigned char *>(srec0 + 2 * rstride);
+    const int tid = threadIdx.x, tile = blockIdx.x, ntiles = P.ntiles;
+    const int istride = kInfoHdr + P.max_halo;
+    const int32_t *info = P.tinfo + (size_t)tile * istride;
+    const int e0 = __ldg(info), ne = __ldg(info + 1), nh = __ldg(info + 2), inflow = __ldg(info + 3);
+    const int nep = (ne + 1) & ~1;
+    const int base = tile * TC, i = base + tid;
+    const double hdry = P.hdry;
+    // ---- everything the tile needs, once per launch
+    for (int q = tid; q < 3 * nep; q += NT) reinterpret_cast<double *>(sedge)[q] = __ldg(P.edges + 3 * (size_t)e0 + q);
+    for (int q = tid; q < 3 * TC; q += NT) scell[q] = __ldg(P.cellc + (size_t)tile * 3 * TC + q);
+    if (tid < TC) {
+        Rec r; r.h = 0.0; r.u = 0.0; r.v = 0.0; r.z = 0.0;
+        if (i < P.nt) r = load_rec(P.U(cur) + i);
+        srec0[tid] = r;
+    }
+    // halo record q of this tile lives in CTA (id / TC) at local index (id % TC)
+    const Rec *hsrc = nullptr;
+    if (tid < nh) {
+        const int id = __ldg(info + kInfoHdr + tid);
+        hsrc = cluster.map_shared_rank(srec0, (unsigned)(id / TC)) + id % TC;
+    }
+    double t_now = __ldcg(&P.ctrl->t[cur]);
+    const double t_end = __ldcg(&P.ctrl->t_end);
+    double dt_cfl = reduce_dt(P, P.pmax(cur), s_red);          // first step: from the rates swe_run left in HBM
+    cluster.sync();                                             // every tile's state is resident
+    double rate = 0.0, dt_last = 0.0;
+    unsigned nclamp = 0, nactive = 0;
+    long long steps = 0;
+    bool all_dry = false;
+    const uint2 *const sab = reinterpret_cast<const uint2 *>(sedge);
+    const double2 *const slxy = reinterpret_cast<const double2 *>(sedge + nep * 8);
+    for (long long s = 0; s < nsteps; s++) {
+        const int p = (int)(s & 1);
+        Rec *const srec = srec0 + p * rstride, *const snew = srec0 + (p ^ 1) * rstride;
+        if (s > 0) {                                            // a11: every CTA holds every tile's maximum
+            double r = 0.0;
+            for (int k = 0; k < ntiles; k++) r = fmax(r, smax[p * kMaxClusterTiles + k]);
+            dt_cfl = r > 0.0 ? P.cfl / r : 0.0;
+        }
+        const double left = t_end - t_now;
+        const bool clipped = dt_cfl >= left;
+        const double dt = fmax(clipped ? left : dt_cfl, 0.0);
+        // a1: halo records from their owners' shared memory
+        bool wet = tid < TC && srec[tid < TC ? tid : 0].h > hdry;
+        if (tid < nh) { const Rec r = hsrc[p * rstride]; srec[TC + tid] = r; wet |= r.h > hdry; }
+        for (int q = tid + NT; q < nh; q += NT) {               // lists longer than the block (poor orderings)
+            const int id = __ldg(info + kInfoHdr + q);
+            const Rec r = *(cluster.map_shared_rank(srec0, (unsigned)(id / TC)) + id % TC + p * rstride);
+            srec[TC + q] = r; wet |= r.h > hdry;
+        }
+        const bool active = __syncthreads_or(wet) || inflow != 0;
+        rate = 0.0;
+        if (!active) {
+            if (tid < TC) snew[tid] = srec[tid];                // all dry: the update is the identity
+        } else {
+            for (int e = tid; e < ne; e += NT) {                // phase 1 (a2-a7)
+                const uint2 ab = sab[e];
+                const double2 l = slxy[e];
+                const Rec A = srec[ab.x & kPosMask];
+                Rec B = A;
+                if ((int32_t)ab.y >= 0) B = srec[ab.y & kPosMask];
+                double o[5];
+                edge_eval(P, l.x, l.y, A, B, (int32_t)ab.y, dt, o);
+                const unsigned sa = ab.x >> kSlotShift;
+                if (sa != kNoSlot) { so01[sa] = make_double2(o[0], o[1]); so2[sa] = o[2]; }
+                const unsigned sb = ab.y >> kSlotShift;
+                if (sb < kNoSlot) { so01[sb] = make_double2(-o[0], -o[3]); so2[sb] = -o[4]; }
+            }
+            __syncthreads();
+            if (tid < TC && i < P.nt) {                         // phase 2 (a7-a10)
+                const Rec Ui = srec[tid];
+                const double2 f0 = so01[tid], f1 = so01[PLC + tid], f2 = so01[2 * PLC + tid];
+                const double s1 = (f0.x + f1.x) + f2.x;
+                const double s2 = (f0.y + f1.y) + f2.y;
+                const double s3 = (so2[tid] + so2[PLC + tid]) + so2[2 * PLC + tid];
+                Rec Un;
+                rate = cell_update(P, Ui, s1, s2, s3, scell[tid], scell[TC + tid], scell[2 * TC + tid], dt, Un, nclamp);
+                snew[tid] = Un;
+            }
+        }
+        rate = block_max(rate, s_red);
+        // this tile's maximum into every CTA's table for the next step (distributed shared memory)
+        if (tid < ntiles) cluster.map_shared_rank(smax, (unsigned)tid)[(p ^ 1) * kMaxClusterTiles + tile] = rate;
+        nactive += active;
+        t_now = clipped ? fmax(t_end, t_now) : t_now + dt;      // R-24
+        if (dt > 0.0) { dt_last = dt; steps++; }
+        if (!(dt_cfl > 0.0)) all_dry = true;
+        cluster.sync();                                         // the step boundary
+    }
+    // ---- back to HBM: state, per-tile maximum, device clock, counters
+    const int fin = cur ^ (int)(nsteps & 1);
+    if (tid < TC && i < P.nt) store_rec(P.U(fin) + i, srec0[(int)(nsteps & 1) * rstride + tid]);
+    if (tid == 0) {
+        P.pmax(fin)[tile] = rate;
+        P.hint[tile] = 1;
+        if (nactive) atomicAdd(&P.ctrl->n_active, (unsigned long long)nactive);
+        if (tile == 0) {
+            Ctrl *c = P.ctrl;
+            c->t[fin] = t_now;
+            if (steps) { c->dt_last = dt_last; c->steps += steps; }
+            if (all_dry) c->all_dry = 1;
+        }
+    }
+    if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);
 }
 
 } // namespace swe

@@ -43,6 +43,7 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
     if (threadIdx.x == 0) {
         uint64_t *bar = reinterpret_cast<uint64_t *>(dyn_smem + SmemLayout<TC>::bar);
         for (int s = 0; s < kNumBars; s++) mbar_init(bar + s, 1);
+        reinterpret_cast<unsigned *>(bar + kNumBars)[0] = 0; reinterpret_cast<unsigned *>(bar + kNumBars)[1] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -54,12 +55,15 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
         const double left = __ldcg(&P.ctrl->t_end) - t_now;
         const bool clipped = dt_cfl >= left;
         const double dt = fmax(clipped ? left : dt_cfl, 0.0);
-        unsigned nclamp = 0, nactive = 0, nelists = 0;
-        double rate = step_tiles<TC>(P, dyn_smem, P.U(cur), P.U(cur ^ 1), dt, nclamp, nactive, nelists, it);
+        unsigned nclamp = 0;
+        double rate = step_tiles<TC>(P, dyn_smem, P.U(cur), P.U(cur ^ 1), dt, nclamp, it);
         rate = block_max(rate, s_red);
         if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
-        if (nactive) atomicAdd(&P.ctrl->n_active, (unsigned long long)nactive);  // likewise (producer thread)
-        if (nelists) atomicAdd(&P.ctrl->n_elists, (unsigned long long)nelists);
+        if (threadIdx.x == TC - 32) {                                            // likewise (the producer thread's counters)
+            unsigned *cnt = reinterpret_cast<unsigned *>(dyn_smem + SmemLayout<TC>::bar) + 2 * kNumBars;
+            if (cnt[0]) { atomicAdd(&P.ctrl->n_active, (unsigned long long)cnt[0]); cnt[0] = 0; }
+            if (cnt[1]) { atomicAdd(&P.ctrl->n_elists, (unsigned long long)cnt[1]); cnt[1] = 0; }
+        }
         if (threadIdx.x == 0) {
             P.pmax(cur ^ 1)[blockIdx.x] = rate;
             if (blockIdx.x == 0) {
@@ -155,7 +159,26 @@ swe_cell_pass_kernel(const Params P, const int cur, const int tile_cells)
     }
 }
 
+// the whole run of a small mesh in one thread-block cluster (cluster_loop, swe_kernels.cuh)
+template <int TC>
+__global__ void __launch_bounds__(2 * TC, 1)
+swe_cluster_kernel(const Params P, int cur, const long long nsteps)
+{
+    __shared__ double s_red[32];
+    cluster_loop<TC>(P, dyn_smem, s_red, cur, nsteps);
+}
+
 typedef void (*step_kernel_t)(const Params, int, const long long);
+step_kernel_t cluster_kernel_for(int tc)
+{
+    switch (tc) {
+    case 64: return swe_cluster_kernel<64>;
+    case 128: return swe_cluster_kernel<128>;
+    case 192: return swe_cluster_kernel<192>;
+    case 256: return swe_cluster_kernel<256>;
+    default: return nullptr;
+    }
+}
 step_kernel_t step_kernel_for(int tc)
 {
     switch (tc) {
@@ -178,7 +201,7 @@ swe_rate_kernel(const Params P, const int cur)
         if (i < P.nt) {
             const Rec U = load_rec(P.U(cur) + i);
             if (U.h > P.hdry)
-                rate = fmax(rate, (sqrt(P.g * U.h) + sqrt(U.u * U.u + U.v * U.v)) *
+                rate = fmax(rate, (sqrt(P.g * U.h) + sqrt(fma(U.u, U.u, U.v * U.v))) *
                                   __ldg(P.cellc + ((size_t)t * 3 + 1) * blockDim.x + threadIdx.x));
         }
     }
@@ -209,7 +232,7 @@ swe_stats_kernel(const Params P, const int cur, const int tile_cells, StatPart *
         const Rec U = load_rec(P.U(cur) + i);
         const int t = (int)(i / tile_cells), q = (int)(i - (long long)t * tile_cells);
         const double area = 1.0 / __ldg(P.cellc + (size_t)t * 3 * tile_cells + q);
-        v += U.h * area;
+        v = fma(U.h, area, v);
         nd += U.h <= P.hdry;
         nb += !(isfinite(U.h) && isfinite(U.u) && isfinite(U.v));
     }
@@ -275,6 +298,8 @@ struct swe_mesh {
     int cur = 0, grid = 0, block = kDefaultBlock, coop_grid = 0, loop_mode = SWE_LOOP_LAUNCH;
     size_t smem = 0;          // dynamic shared memory of the step kernel
     void (*kern)(const Params, int, const long long) = nullptr;
+    void (*ckern)(const Params, int, const long long) = nullptr;   // SWE_LOOP_CLUSTER
+    size_t csmem = 0;
     int64_t launches = 0;
     double qn_tag[SWE_BC_MAX_TAG + 1] = {};
     std::map<std::pair<int, int>, cudaGraphExec_t> graphs; // (steps, cur) -> exec
@@ -349,7 +374,7 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     swe_params_default(&p);
     if (params) p = *params;
     if (!(p.g > 0.0) || !(p.cfl > 0.0) || !(p.h_dry >= 0.0) || p.ordering < 0 || p.ordering > SWE_ORDER_RCM ||
-        p.loop_mode < 0 || p.loop_mode > SWE_LOOP_LAUNCH || p.riemann < 0 || p.riemann > SWE_RIEMANN_HLL ||
+        p.loop_mode < 0 || p.loop_mode > SWE_LOOP_CLUSTER || p.riemann < 0 || p.riemann > SWE_RIEMANN_HLL ||
         p.kernel < 0 || p.kernel > SWE_KERNEL_EDGE_TWO_PASS ||
         (p.block_size != 0 && p.block_size != 64 && p.block_size != 128 && p.block_size != 192 && p.block_size != 256)) {
         g_create_err = "swe_mesh_create: invalid swe_params (block_size must be 0, 64, 128, 192 or 256)";
@@ -364,6 +389,10 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     } catch (const std::bad_alloc &) { rc = SWE_ERR_NOMEM; m->err = "out of host memory"; }
     if (rc != SWE_OK) { g_create_err = m->err; delete m; return rc; }
     m->block = p.block_size ? p.block_size : kDefaultBlock;
+    // small meshes that AUTO will run as one cluster: 128-cell tiles (up to 16 of them)
+    if (!p.block_size && p.kernel == SWE_KERNEL_TILED && (p.loop_mode == SWE_LOOP_AUTO || p.loop_mode == SWE_LOOP_CLUSTER) &&
+        nt <= (int64_t)kMaxClusterTiles * 128)
+        m->block = 128;
     rc = build_tiles(m->T, m->block, p.g, m->X, m->err);
     if (rc != SWE_OK) { g_create_err = m->err; delete m; return rc; }
     m->edge_kernel = p.kernel == SWE_KERNEL_EDGE_TWO_PASS;
@@ -542,7 +571,26 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     // measured on B200 (2000 to 200 000 cells): replaying 128-step CUDA graphs is as fast as the
     // cooperative launch on the smallest meshes (6.0 us per step at 11 blocks) and 14 % faster once
     // blocks own two tiles (12.8 vs 14.9 us at 200 000 cells), so AUTO means GRAPH
-    if (mode == SWE_LOOP_AUTO) mode = SWE_LOOP_GRAPH;
+    if ((mode == SWE_LOOP_AUTO || mode == SWE_LOOP_CLUSTER) && !m->edge_kernel && ntiles <= kMaxClusterTiles) {
+        // can one cluster of ntiles CTAs be resident?  (non-portable sizes above 8 need the opt-in)
+        m->ckern = cluster_kernel_for(m->block);
+        m->csmem = cluster_smem_bytes(m->block, X.max_halo, X.max_edges);
+        int nclusters = 0;
+        if (m->csmem <= (size_t)smem_optin - 1024 &&
+            cudaFuncSetAttribute((const void *)m->ckern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin - 1024) == cudaSuccess &&
+            cudaFuncSetAttribute((const void *)m->ckern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(ntiles); cfg.blockDim = dim3(2 * m->block); cfg.dynamicSmemBytes = m->csmem;
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = ntiles; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.attrs = at; cfg.numAttrs = 1;
+            if (cudaOccupancyMaxActiveClusters(&nclusters, (const void *)m->ckern, &cfg) != cudaSuccess) nclusters = 0;
+        }
+        (void)cudaGetLastError();
+        mode = nclusters >= 1 ? SWE_LOOP_CLUSTER : SWE_LOOP_GRAPH;
+    }
+    if (mode == SWE_LOOP_AUTO || mode == SWE_LOOP_CLUSTER) mode = mode == SWE_LOOP_CLUSTER && m->ckern && ntiles <= kMaxClusterTiles && !m->edge_kernel ? mode : SWE_LOOP_GRAPH;
     if (mode == SWE_LOOP_PERSISTENT && !coop) mode = SWE_LOOP_GRAPH;
     if (m->edge_kernel) {
         // two kernels per step: the kernel boundary is the only grid-wide barrier they have
@@ -760,6 +808,18 @@ int swe_run(swe_mesh *m, int64_t nsteps)
         Params P = m->P; int cur = m->cur; long long ns = nsteps;
         void *args[] = { &P, &cur, &ns };
         CK(cudaLaunchCooperativeKernel((void *)m->kern, dim3(m->coop_grid), dim3(m->block), args, m->smem, m->stream));
+        m->launches++;
+        m->cur ^= (int)(nsteps & 1);
+        return SWE_OK;
+    }
+    if (m->loop_mode == SWE_LOOP_CLUSTER) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(m->grid); cfg.blockDim = dim3(2 * m->block); cfg.dynamicSmemBytes = m->csmem; cfg.stream = m->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = m->grid; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        CK(cudaLaunchKernelEx(&cfg, m->ckern, m->P, m->cur, (long long)nsteps));
         m->launches++;
         m->cur ^= (int)(nsteps & 1);
         return SWE_OK;

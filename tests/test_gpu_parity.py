@@ -48,7 +48,7 @@ def assert_parity(m, o, w):
     return hg, hug, hvg, tg
 
 
-LOOPS = [B.LOOP_GRAPH, B.LOOP_PERSISTENT, B.LOOP_LAUNCH]
+LOOPS = [B.LOOP_GRAPH, B.LOOP_PERSISTENT, B.LOOP_LAUNCH, B.LOOP_CLUSTER]
 
 
 @pytest.mark.parametrize("loop_mode", LOOPS)
@@ -141,6 +141,44 @@ def test_determinism_and_loop_modes_bitwise():
             for a, b in zip(ref[:3], got[:3]):
                 np.testing.assert_array_equal(a, b)
             assert ref[3] == got[3] and ref[4] == got[4]
+
+
+def test_cluster_loop_bitwise_equal_to_the_other_loop_modes():
+    """Small meshes (<= 16 tiles): one thread-block cluster runs the whole swe_run with the state in
+    shared memory, halo records through distributed shared memory and the cluster barrier per step.
+    Same bits as the graph / persistent loops (different tile size included), AUTO picks it, and a
+    run split into several calls (state written back and reloaded) changes nothing."""
+    for w in (W.config1(), W.config4(nx=40, ny=10), W.canal_dam_break(37, 7, seed=9, length=37.0, manning=0.02, h_right=0.0)):
+        ref = None
+        for loop_mode, block in ((B.LOOP_GRAPH, 192), (B.LOOP_PERSISTENT, 128), (B.LOOP_CLUSTER, 0), (B.LOOP_AUTO, 0),
+                                 (B.LOOP_CLUSTER, 192), (B.LOOP_CLUSTER, 256)):
+            m = B.SweMesh.from_workload(w, loop_mode=loop_mode, block_size=block).bind_device()
+            m.set_state(w.h, w.hu, w.hv)
+            m.run(137); m.run(64); m.step()
+            got = m.get_state()
+            info = m.get_launch_info()
+            if loop_mode in (B.LOOP_CLUSTER, B.LOOP_AUTO):
+                assert info["loop_mode"] == "cluster" and info["block"] == (block or 128)
+            if ref is None:
+                ref = got
+                vol = m.get_boundary_volumes()
+            else:
+                for a, b in zip(ref[:3], got[:3]):
+                    np.testing.assert_array_equal(a, b)
+                assert ref[3] == got[3] and ref[4] == got[4]
+                np.testing.assert_array_equal(vol, m.get_boundary_volumes())
+                assert m.get_stats()["steps"] == 202
+    # run_until in cluster mode ends on t_end exactly, in as many steps as the oracle
+    w = W.config1()
+    m = B.SweMesh.from_workload(w, loop_mode=B.LOOP_CLUSTER).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    o = OracleSolver.from_workload(w)
+    assert m.run_until(2.0) == o.run_until(2.0)
+    assert m.get_state()[3] == 2.0
+    # a mesh with more than 16 tiles falls back to the graph loop
+    w = W.config2(nx=100, ny=20)
+    m = B.SweMesh.from_workload(w, loop_mode=B.LOOP_CLUSTER).bind_device()
+    assert m.get_launch_info()["loop_mode"] == "graph"
 
 
 def test_edge_cases():
@@ -260,8 +298,7 @@ def test_edge_two_pass_kernel_matches_oracle_and_tiled_kernel(loop_mode):
     """Pass 1 (one thread per edge of the mesh) + pass 2 (one thread per cell): the same scheme as
     the fused tile kernel, against the oracle at the same bar, river case with inflow / outflow /
     wet-dry fronts / friction; and against the tile kernel itself (same edge and cell arithmetic,
-    same order k = 0,1,2; the compiler contracts the two instantiations differently, so they agree
-    to round-off, not to the bit)."""
+    same order k = 0,1,2, every fused multiply-add written out and --fmad=false: identical bits)."""
     w = W.config4(nx=320, ny=80)
     m, o = run_both(w, 600, kernel=B.KERNEL_EDGE_TWO_PASS, loop_mode=loop_mode)
     got = assert_parity(m, o, w)
@@ -271,8 +308,8 @@ def test_edge_two_pass_kernel_matches_oracle_and_tiled_kernel(loop_mode):
     r.run(600)
     ref = r.get_state()
     for a, b in zip(got[:3], ref[:3]):
-        np.testing.assert_allclose(a, b, rtol=1e-12, atol=1e-12)
-    assert got[3] == pytest.approx(ref[3], rel=1e-14)
+        np.testing.assert_array_equal(a, b)
+    assert got[3] == ref[3]
 
 
 def test_edge_two_pass_kernel_ordering_invariance_and_run_until():
