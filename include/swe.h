@@ -107,6 +107,9 @@ typedef struct {
     int64_t edge_list_fetches; /* sum over the steps of the number of tile edge lists read from HBM (the list of
                                   a tile that was all dry at the previous step is read only if the tile turns
                                   out active): with active_tile_steps it fixes the bytes a step requests */
+    int64_t quiet_tile_steps;  /* sum over the steps of the number of QUIET tiles: inactive in the previous step with
+                                  all their neighbour tiles, hence all dry now; their records are copied through
+                                  registers without a halo gather or a vote */
 } swe_stats;
 
 /* Fills *p with the defaults listed above. */
@@ -260,15 +263,18 @@ int swe_get_tile_info(const swe_mesh *mesh, int32_t *tile_cells, int64_t *ntiles
 
 /*
  * Bytes one time step REQUESTS from device memory, from the library's own table sizes, given how
- * many tiles are active (not all dry) and how many tile edge lists are fetched in that step (both
- * may be per-step averages taken from swe_stats.active_tile_steps / edge_list_fetches): every cell's
- * 32-byte record in and out, one 32-byte sector per halo record, tile headers + halo ids + hints,
+ * many tiles are active (not all dry), how many tile edge lists are fetched and how many tiles are
+ * quiet (copied without a halo gather) in that step (per-step averages taken from swe_stats.
+ * active_tile_steps / edge_list_fetches / quiet_tile_steps): every cell's 32-byte record in and
+ * out, one 32-byte sector per halo record of a tile that is not quiet, tile headers + halo ids,
+ * activity flags and neighbour-tile rows,
  * 24 bytes of cell constants per cell of an active tile, 24 bytes per edge of a fetched list (mean
  * list length).  This is the kernel's request stream, not a DRAM counter: L2 hits on the halo
  * records make the DRAM traffic smaller (bench.py reports it as roofline.traffic; the cross-check
  * against ncu's dram__bytes is in profiles/).
  */
-int swe_get_step_bytes(const swe_mesh *mesh, double active_tiles, double edge_lists, double *bytes);
+int swe_get_step_bytes(const swe_mesh *mesh, double active_tiles, double edge_lists, double quiet_tiles,
+                       double *bytes);
 
 /*
  * The tile tables themselves, for tests of the mesh builder; any pointer may be NULL.

@@ -44,7 +44,7 @@ class SweStats(C.Structure):
     _fields_ = [("volume", C.c_double), ("t", C.c_double), ("dt_last", C.c_double),
                 ("steps", C.c_int64), ("n_dry", C.c_int64), ("n_clamped", C.c_int64),
                 ("n_nonfinite", C.c_int64), ("active_tile_steps", C.c_int64),
-                ("edge_list_fetches", C.c_int64)]
+                ("edge_list_fetches", C.c_int64), ("quiet_tile_steps", C.c_int64)]
 
 
 class SweError(RuntimeError):
@@ -93,7 +93,7 @@ def load_library(rebuild_if_stale: bool = True):
                                     C.POINTER(C.c_size_t)]
     L.swe_get_tile_tables.argtypes = [vp, i32p, i32p, dp, i32p]
     L.swe_get_launch_info.argtypes = [vp, i32p, i32p, i32p, C.POINTER(C.c_int64)]
-    L.swe_get_step_bytes.argtypes = [vp, C.c_double, C.c_double, dp]
+    L.swe_get_step_bytes.argtypes = [vp, C.c_double, C.c_double, C.c_double, dp]
     L.swe_last_error.argtypes = [vp]
     L.swe_last_error.restype = C.c_char_p
     for name in SYMBOLS:
@@ -312,9 +312,10 @@ class SweMesh:
                                              _dp(geom), tinfo.ctypes.data_as(i32p)))
         return dict(edge_a=a, edge_b=b, edge_geom=geom, tinfo=tinfo, **ti)
 
-    def get_step_bytes(self, active_tiles, edge_lists) -> float:
+    def get_step_bytes(self, active_tiles, edge_lists, quiet_tiles=0.0) -> float:
         b = C.c_double(0.0)
-        self._ck(self._L.swe_get_step_bytes(self._h, float(active_tiles), float(edge_lists), C.byref(b)))
+        self._ck(self._L.swe_get_step_bytes(self._h, float(active_tiles), float(edge_lists), float(quiet_tiles),
+                                            C.byref(b)))
         return b.value
 
     def get_launch_info(self) -> dict:

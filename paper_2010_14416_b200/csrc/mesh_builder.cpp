@@ -550,6 +550,23 @@ int build_tiles(const HostTables &T, int tile_cells, double g, TileTables &X, st
                 if (X.edges[(size_t)e].b < 0 && ((-X.edges[(size_t)e].b) & 127) >= SWE_BC_INFLOW0) ti[3] = 1;  // prescribed discharge
             std::copy(halo.begin() + hstart[(size_t)t], halo.begin() + hstart[(size_t)t + 1], ti + 4);
         }
+        // the tiles that own each tile's halo cells (distinct, in order of first appearance)
+        X.tnbr.assign((size_t)X.ntiles * kTileNbrs, -1);
+        parallel_for(X.ntiles, [&](int64_t tb, int64_t te, int) {
+            for (int64_t t = tb; t < te; t++) {
+                int32_t *row = X.tnbr.data() + (size_t)t * kTileNbrs;
+                int cnt = 0; bool never = X.tinfo[(size_t)t * stride + 3] != 0;       // prescribed discharge
+                for (int32_t h = hstart[(size_t)t]; h < hstart[(size_t)t + 1] && !never; h++) {
+                    const int32_t owner = halo[(size_t)h] / TC;
+                    bool seen = false;
+                    for (int q = 0; q < cnt; q++) seen |= row[q] == owner;
+                    if (seen) continue;
+                    if (cnt == kTileNbrs) { never = true; break; }
+                    row[cnt++] = owner;
+                }
+                if (never) { std::fill(row, row + kTileNbrs, -1); row[0] = -2; }
+            }
+        }, 1024);
     } catch (const std::bad_alloc &) { err = "out of host memory"; return SWE_ERR_NOMEM; }
     return SWE_OK;
 }

@@ -38,6 +38,7 @@ struct HostTables {
 // records (a zero record) so that every tile's list starts and ends on a 16-byte boundary.
 struct HostEdge { int32_t a, b; double lx, ly; };                               // 24 bytes
 constexpr int kHostIdBits = 29;
+constexpr int kTileNbrs = 16;
 struct TileTables {
     int32_t tile_cells = 0;
     int64_t ntiles = 0;
@@ -45,6 +46,9 @@ struct TileTables {
     int64_t nedges = 0;                // edge records without the padding
     int32_t max_halo = 0;              // longest halo list of any tile, rounded up to a multiple of 4
     int64_t nhalo = 0;                 // halo entries of all tiles together
+    // [ntiles][kTileNbrs] the tiles that own this tile's halo cells, padded with -1; tnbr[t][0] = -2 if
+    // the tile has more than kTileNbrs such neighbours or an inflow edge ("never quiet", swe_kernels.cuh)
+    std::vector<int32_t> tnbr;
     // [ntiles][4 + max_halo]: {first edge, #edges, #halo ids, 1 if the tile has an inflow edge else 0,
     // halo ids (internal cell ids of the tile's off-tile end points) padded with -1}
     std::vector<int32_t> tinfo;

@@ -74,6 +74,7 @@ struct Ctrl {                 // device-resident loop state
     unsigned long long n_clamped;
     unsigned long long n_active;  // tiles that were not all dry, summed over the steps (diagnostics)
     unsigned long long n_elists;  // edge lists fetched, summed over the steps (diagnostics)
+    unsigned long long n_quiet;   // quiet tiles (copied through registers), summed over the steps (diagnostics)
     int all_dry;              // set when a step found no wet cell
     int bad_cell;             // smallest caller id with a negative depth or a non-finite value (swe_set_state)
 };
@@ -85,7 +86,9 @@ struct Params {
     const int32_t *tinfo;     // [ntiles][4 + max_halo] per-tile header + halo ids, see "the tile pipeline"
     const double *qn_tag;     // [128] unit discharge along the outward normal per inflow tag
     double *bvol;             // [boundary edges] cumulative outward volume through each boundary edge
-    int32_t *hint;            // [ntiles] 1 if the tile was active (not all dry) at the previous step
+    int32_t *act0, *act1;     // [ntiles] 1 if the tile was active (not all dry) in the step that produced U0 / U1
+    const int32_t *tnbr;      // [ntiles][kNbrs] tiles owning each tile's halo cells (-1 padding; [0] = -2: never quiet)
+    int32_t *binact;          // [npart] inactive tiles of each block's sequence in the previous step
     double *pmax0, *pmax1;    // [npart] per-block max rate of state U0 / U1
     Ctrl *ctrl;
     // edge-centric two-pass kernels only (SWE_KERNEL_EDGE_TWO_PASS; NULL otherwise)
@@ -99,6 +102,7 @@ struct Params {
     // selected with a ternary so the kernel parameter block is never indexed dynamically
     __host__ __device__ __forceinline__ Rec *U(int c) const { return c ? U1 : U0; }
     __host__ __device__ __forceinline__ double *pmax(int c) const { return c ? pmax1 : pmax0; }
+    __host__ __device__ __forceinline__ int32_t *act(int c) const { return c ? act1 : act0; }
 };
 
 // ---- 256-bit access --------------------------------------------------------------------------
@@ -493,13 +497,16 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 //   phase 2  cells
 constexpr int kInfoHdr = 4;
 constexpr int kNumBars = 5;
+constexpr int kMaxSeq = 4096;             // tiles of a block's sequence that can be flagged quiet (the rest vote)
+constexpr int kNbrs = 16;                 // = kTileNbrs (mesh_builder.h)
 template <int TC> struct SmemLayout {
     static constexpr int PLC = TC + 1;
     static constexpr int so01 = 0;
     static constexpr int so2 = so01 + 3 * PLC * 16;
     static constexpr int scell = (so2 + 3 * PLC * 8 + 15) & ~15;
     static constexpr int bar = scell + 3 * TC * 8;
-    static constexpr int srec = (bar + kNumBars * 8 + 8 + 31) & ~31;     // + two diagnostic counters
+    static constexpr int sq = bar + kNumBars * 8 + 16;                   // after four diagnostic counters
+    static constexpr int srec = (sq + kMaxSeq / 8 + 31) & ~31;
 };
 __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int ME)
 {
@@ -507,7 +514,7 @@ __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int M
     size_t o = 3 * PLC * 16;
     o = (o + 3 * PLC * 8 + 15) & ~(size_t)15;
     o += 3 * (size_t)TC * 8;
-    o = (o + kNumBars * 8 + 8 + 31) & ~(size_t)31;
+    o = (o + kNumBars * 8 + 16 + 4096 / 8 + 31) & ~(size_t)31;           // barriers, counters, quiet flags (kMaxSeq bits)
     o += 2 * (size_t)(TC + MH) * sizeof(Rec);
     o += 2 * (size_t)ME * 24;
     return o;
@@ -518,21 +525,126 @@ __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int M
 // not complete a phase at every tile (edge lists: one bit per stage; cell constants).
 struct PipeState { unsigned n = 0, epar = 0, cpar = 0; };
 
+// ---- quiet tiles -------------------------------------------------------------------------------------
+// P.act(c)[t] = 1 if tile t was active (not all dry) in the step that produced the state in U(c).  A
+// tile that was inactive in the previous step, and whose halo cells all belong to tiles that were
+// inactive in the previous step too, is QUIET: none of its cells and none of its halo cells has
+// changed since they were seen dry, so it is all dry now, and its update is the identity whatever
+// its neighbours do in this step.  A quiet tile needs no halo gather, no vote, no shared memory: its
+// records go from U(cur) to U(cur^1) through registers, four tiles in flight per thread, which is
+// what keeps HBM busy on the dry part of a mesh (the paper's river domains are mostly dry land).
+// Tiles with an inflow edge or with more than kTileNbrs neighbour tiles are never quiet (tnbr[0] = -2).
+// The block's tiles are tile(j) = blockIdx.x + j gridDim.x; bit j of sq[] says tile(j) is quiet.
+
+// one flag per tile of the block's sequence, evaluated by one thread each (17 words from L2)
+template <int TC>
+__device__ __forceinline__ void quiet_flags(const Params &P, const int32_t *__restrict__ act_prev, unsigned *sq, const int nmy)
+{
+    const int tid = threadIdx.x, G = gridDim.x, lim = min(nmy, kMaxSeq);
+    for (int j0 = 0; j0 < lim; j0 += TC) {
+        const int j = j0 + tid;
+        int v = 1;
+        if (j < lim) {
+            const int t = blockIdx.x + j * G;
+            v = ldcg_i32(act_prev + t);
+            if (v == 0) {
+                const int4 *row = reinterpret_cast<const int4 *>(P.tnbr + (size_t)t * kNbrs);
+#pragma unroll
+                for (int q = 0; q < kNbrs / 4; q++) {
+                    const int4 r = __ldg(row + q);
+                    v |= r.x == -2;
+                    if (r.x >= 0) v |= ldcg_i32(act_prev + r.x);
+                    if (r.y >= 0) v |= ldcg_i32(act_prev + r.y);
+                    if (r.z >= 0) v |= ldcg_i32(act_prev + r.z);
+                    if (r.w >= 0) v |= ldcg_i32(act_prev + r.w);
+                }
+            }
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, v == 0);
+        if ((tid & 31) == 0 && j < ((lim + 31) & ~31)) sq[j >> 5] = m;
+    }
+}
+__device__ __forceinline__ int next_nonquiet(const unsigned *sq, int j, const int nmy)
+{
+    const int lim = min(nmy, kMaxSeq);
+    while (j < lim) {
+        const unsigned w = ~sq[j >> 5] & (0xffffffffu << (j & 31));
+        if (w) return min((j & ~31) + __ffs(w) - 1, nmy);
+        j = (j | 31) + 1;
+    }
+    return min(j, nmy);
+}
+__device__ __forceinline__ int next_quiet(const unsigned *sq, int j, const int nmy)
+{
+    const int lim = min(nmy, kMaxSeq);
+    while (j < lim) {
+        const unsigned w = sq[j >> 5] & (0xffffffffu << (j & 31));
+        if (w) { j = (j & ~31) + __ffs(w) - 1; return j < lim ? j : nmy; }
+        j = (j | 31) + 1;
+    }
+    return nmy;
+}
+// every quiet tile of the block's sequence: records from U(cur) to U(cur^1) through registers, four
+// tiles in flight per thread; returns how many there were
+// (out of line, called once per step before the tile loop: its registers are its own)
+template <int TC>
+__device__ __noinline__ int copy_quiet_tiles(const int nt, const unsigned *sq, const Rec *__restrict__ Uin,
+                                             Rec *__restrict__ Uout, int32_t *__restrict__ act_next, const int nmy)
+{
+    const int tid = threadIdx.x, G = gridDim.x;
+    int count = 0;
+    int j = next_quiet(sq, 0, nmy);
+    while (j < nmy) {
+        // (named variables, not arrays: the four records must stay in registers)
+        int t0 = -1, t1 = -1, t2 = -1, t3 = -1;
+        t0 = blockIdx.x + j * G; j = next_quiet(sq, j + 1, nmy); count++;
+        if (j < nmy) { t1 = blockIdx.x + j * G; j = next_quiet(sq, j + 1, nmy); count++; }
+        if (j < nmy) { t2 = blockIdx.x + j * G; j = next_quiet(sq, j + 1, nmy); count++; }
+        if (j < nmy) { t3 = blockIdx.x + j * G; j = next_quiet(sq, j + 1, nmy); count++; }
+        const long long i0 = (long long)t0 * TC + tid, i1 = (long long)t1 * TC + tid;
+        const long long i2 = (long long)t2 * TC + tid, i3 = (long long)t3 * TC + tid;
+        const bool p0 = i0 < nt, p1 = t1 >= 0 && i1 < nt, p2 = t2 >= 0 && i2 < nt, p3 = t3 >= 0 && i3 < nt;
+        // (unconditional loads from a valid address: a conditional one would put the record in local memory)
+        const Rec r0 = load_rec(Uin + (p0 ? i0 : 0)), r1 = load_rec(Uin + (p1 ? i1 : 0));
+        const Rec r2 = load_rec(Uin + (p2 ? i2 : 0)), r3 = load_rec(Uin + (p3 ? i3 : 0));
+        if (p0) store_rec(Uout + i0, r0);
+        if (p1) store_rec(Uout + i1, r1);
+        if (p2) store_rec(Uout + i2, r2);
+        if (p3) store_rec(Uout + i3, r3);
+        if (tid == 0) {
+            act_next[t0] = 0;
+            if (t1 >= 0) act_next[t1] = 0;
+            if (t2 >= 0) act_next[t2] = 0;
+            if (t3 >= 0) act_next[t3] = 0;
+        }
+    }
+    return count;
+}
+
 // All the tiles of this block for one time step.
 // Returns this thread's maximum rate contribution.
-template <int TC>
-__device__ __forceinline__ double step_tiles(const Params &P, unsigned char *smem,
-                                             const Rec *__restrict__ Uin, Rec *__restrict__ Uout,
+// QUIET: look for quiet tiles and copy them through registers first (chosen per block and step when
+// a good share of the block's tiles was inactive in the previous step; the results are the same
+// either way, an all-dry tile that is not treated as quiet is found by the vote).
+template <int TC, bool QUIET>
+__device__ __forceinline__ double step_tiles(const Params &P, unsigned char *smem, const int cur,
                                              const double dt, unsigned &nclamp, PipeState &ps)
 {
+    // state and activity flags of this step: read side cur, written side cur ^ 1.  The pointers are
+    // re-derived from the kernel parameters where they are used (registers are what limits the tile loop)
+#define Uin (static_cast<const Rec *>(P.U(cur)))
+#define Uout (P.U(cur ^ 1))
+#define act_prev (static_cast<const int32_t *>(P.act(cur)))
+#define act_next (P.act(cur ^ 1))
     typedef SmemLayout<TC> SL;
     constexpr int PLC = SL::PLC;
     double2 *const so01 = reinterpret_cast<double2 *>(smem + SL::so01);
     double *const so2 = reinterpret_cast<double *>(smem + SL::so2);
     const double *const scell = reinterpret_cast<const double *>(smem + SL::scell);
     uint64_t *const bar = reinterpret_cast<uint64_t *>(smem + SL::bar);      // rec 0,1; edge 2,3; cell 4
-    // diagnostics kept by the producer thread: [0] active tiles, [1] edge lists fetched (this launch)
+    // kept by the producer thread: [0] active tiles, [1] edge lists fetched, [2] quiet tiles, [3] inactive tiles
     volatile unsigned *const scount = reinterpret_cast<volatile unsigned *>(bar + kNumBars);
+    unsigned *const sq = reinterpret_cast<unsigned *>(smem + SL::sq);        // quiet flags of the block's tiles
     Rec *const srec0 = reinterpret_cast<Rec *>(smem + SL::srec);
     const int rstride = TC + P.max_halo;
     unsigned char *const sedge0 = reinterpret_cast<unsigned char *>(srec0 + 2 * rstride);
@@ -541,8 +653,8 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
     const int tid = threadIdx.x, G = gridDim.x;
     const double hdry = P.hdry;
     double rate = 0.0;
-    int tile = blockIdx.x;
-    if (tile >= P.ntiles) return 0.0;
+    if ((int)blockIdx.x >= P.ntiles) return 0.0;
+    const int nmy = (P.ntiles - (int)blockIdx.x + G - 1) / G;       // tiles of this block: tile(j) = blockIdx.x + j G
     unsigned n = ps.n, epar = ps.epar, cpar = ps.cpar;
     // the copies are issued by lane 0 of the LAST warp: the edge loop gives the first warps one more
     // iteration than the last ones (ne ~ 1.66 TC), so the last warp has the slack
@@ -582,22 +694,35 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
     auto hdr_ne = [](int4 h) { return h.y; };
     auto hdr_nh = [](int4 h) { return h.z; };
     auto load_hid = [&](int t) { return tid < P.max_halo ? __ldg(P.tinfo + (size_t)t * istride + kInfoHdr + tid) : -1; };
+    auto tile_of = [&](int j) { return (int)blockIdx.x + j * G; };
 
-    // ---- prologue: everything tile n needs; header, halo id and hint of tile n+1
-    int4 hdr0 = load_hdr(tile), hdr1 = make_int4(0, 0, 0, 0);
-    int hid0 = load_hid(tile), hid1 = -1, hint1 = 0;
-    bool req0 = true;                    // was this tile's edge list requested?  The step's first tile: always
+    // ---- which of this block's tiles are quiet; the pipeline below runs over the others
+    auto next_stage = [&](int j) { if constexpr (QUIET) return next_nonquiet(sq, j, nmy); else return min(j, nmy); };
+    if constexpr (QUIET) {
+        quiet_flags<TC>(P, act_prev, sq, nmy);
+        __syncthreads();
+        const int nq = copy_quiet_tiles<TC>(P.nt, sq, Uin, Uout, act_next, nmy);
+        if (producer) { scount[2] += (unsigned)nq; scount[3] += (unsigned)nq; }
+    }
+    int j0 = next_stage(0);                              // this pipeline stage, the next one, the one after
+    int j1 = j0 < nmy ? next_stage(j0 + 1) : nmy;
+    if (j0 >= nmy) return 0.0;                           // nothing but quiet tiles
+    // ---- prologue: everything tile(j0) needs; header, halo id and hint of tile(j1)
+    int4 hdr0 = load_hdr(tile_of(j0)), hdr1 = make_int4(0, 0, 0, 0);
+    int hid0 = load_hid(tile_of(j0)), hid1 = -1, hint1 = 0;
+    bool req0 = true;                    // was this tile's edge list requested?  The step's first pipeline stage: always
     if (producer) {
-        issue_recs(tile, n & 1);
+        issue_recs(tile_of(j0), n & 1);
         issue_edges(hdr0.x, hdr_ne(hdr0), n & 1);
     }
-    if (tile + G < P.ntiles) { hdr1 = load_hdr(tile + G); hid1 = load_hid(tile + G); hint1 = ldcg_i32(P.hint + tile + G); }
-    gather_halo(tile, hdr_nh(hdr0), hid0, n & 1);
+    if (j1 < nmy) { hdr1 = load_hdr(tile_of(j1)); hid1 = load_hid(tile_of(j1)); hint1 = ldcg_i32(act_prev + tile_of(j1)); }
+    gather_halo(tile_of(j0), hdr_nh(hdr0), hid0, n & 1);
     cp_async_commit();
     for (;;) {
         const int s = n & 1;
+        const int tile = tile_of(j0);
         const int base = tile * TC;
-        const bool have_next = tile + G < P.ntiles;
+        const bool have_next = j1 < nmy;
         const int ne = hdr_ne(hdr0), nh = hdr_nh(hdr0);
         // ---- top
         cp_async_wait<0>();                               // own halo gathers of this tile
@@ -613,7 +738,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
         const bool active = __syncthreads_or(wet) || hdr0.w != 0;
         if (producer) {
             if (have_next) {
-                issue_recs(tile + G, s ^ 1);
+                issue_recs(tile_of(j1), s ^ 1);
                 // Edge lists are 40 of the ~105 bytes a cell costs and an all-dry tile never reads its
                 // list, so the list of the NEXT tile is requested only if that tile was active at the
                 // previous step; a tile that turns out active without its list (the wet front reached
@@ -621,16 +746,16 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
                 if (hint1) issue_edges(hdr1.x, hdr_ne(hdr1), s ^ 1);
             }
             if (active) issue_cellc(tile);
-            P.hint[tile] = active;
-            scount[0] += active;
+            act_next[tile] = active;
+            scount[0] += active; scount[3] += !active;
         }
-        if (have_next) gather_halo(tile + G, hdr_nh(hdr1), hid1, s ^ 1);
+        if (have_next) gather_halo(tile_of(j1), hdr_nh(hdr1), hid1, s ^ 1);
         cp_async_commit();
+        // the stage after the next one: its header, halo id and hint into registers
+        const int j2 = have_next ? next_stage(j1 + 1) : nmy;
         int4 hdr2 = make_int4(0, 0, 0, 0);
         int hid2 = -1, hint2 = 0;
-        if (tile + 2 * G < P.ntiles) {
-            hdr2 = load_hdr(tile + 2 * G); hid2 = load_hid(tile + 2 * G); hint2 = ldcg_i32(P.hint + tile + 2 * G);
-        }
+        if (j2 < nmy) { hdr2 = load_hdr(tile_of(j2)); hid2 = load_hid(tile_of(j2)); hint2 = ldcg_i32(act_prev + tile_of(j2)); }
         // this tile's edge list: requested one tile ago, or fetched now if the tile is active without it
         if (!req0 && active && producer) issue_edges(hdr0.x, ne, s);
         if (req0 || active) {
@@ -684,13 +809,18 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
             }
         }
         if (!have_next) break;
-        tile += G; n++;
+        n++;
+        j0 = j1; j1 = j2;
         hdr0 = hdr1; hid0 = hid1; req0 = hint1 != 0;
         hdr1 = hdr2; hid1 = hid2; hint1 = hint2;
     }
     cp_async_wait<0>();
     ps.n = n + 1; ps.epar = epar; ps.cpar = cpar;
     return rate;
+#undef Uin
+#undef Uout
+#undef act_prev
+#undef act_next
 }
 
 // ---- small meshes: the whole time loop in ONE thread-block cluster ---------------------------------
@@ -831,7 +961,6 @@ __device__ __forceinline__ void cluster_loop(const Params &P, unsigned char *sme
     if (tid < TC && i < P.nt) store_rec(P.U(fin) + i, srec0[(int)(nsteps & 1) * rstride + tid]);
     if (tid == 0) {
         P.pmax(fin)[tile] = rate;
-        P.hint[tile] = 1;
         if (nactive) atomicAdd(&P.ctrl->n_active, (unsigned long long)nactive);
         if (tile == 0) {
             Ctrl *c = P.ctrl;

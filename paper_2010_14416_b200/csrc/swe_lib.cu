@@ -43,12 +43,13 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
     if (threadIdx.x == 0) {
         uint64_t *bar = reinterpret_cast<uint64_t *>(dyn_smem + SmemLayout<TC>::bar);
         for (int s = 0; s < kNumBars; s++) mbar_init(bar + s, 1);
-        reinterpret_cast<unsigned *>(bar + kNumBars)[0] = 0; reinterpret_cast<unsigned *>(bar + kNumBars)[1] = 0;
+        for (int q = 0; q < 4; q++) reinterpret_cast<unsigned *>(bar + kNumBars)[q] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     PipeState it;
     for (long long s = 0; s < nsteps; s++) {
+        const int ninact = ldcg_i32(P.binact + blockIdx.x);      // (in flight during the reduction below)
         const double dt_cfl = reduce_dt(P, P.pmax(cur), s_red);
         // swe_run_until: the step that would pass t_end ends on it; after that, zero steps
         const double t_now = __ldcg(&P.ctrl->t[cur]);
@@ -56,13 +57,19 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
         const bool clipped = dt_cfl >= left;
         const double dt = fmax(clipped ? left : dt_cfl, 0.0);
         unsigned nclamp = 0;
-        double rate = step_tiles<TC>(P, dyn_smem, P.U(cur), P.U(cur ^ 1), dt, nclamp, it);
+        // quiet tiles are looked for when at least a quarter of the block's tiles were inactive a step ago
+        // and the block has enough tiles to repay the look (flags, a barrier, the scan)
+        const int nmy = (int)blockIdx.x < P.ntiles ? (P.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+        double rate = 4 * ninact >= nmy && nmy >= 8 ? step_tiles<TC, true>(P, dyn_smem, cur, dt, nclamp, it)
+                                                      : step_tiles<TC, false>(P, dyn_smem, cur, dt, nclamp, it);
         rate = block_max(rate, s_red);
         if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
         if (threadIdx.x == TC - 32) {                                            // likewise (the producer thread's counters)
             unsigned *cnt = reinterpret_cast<unsigned *>(dyn_smem + SmemLayout<TC>::bar) + 2 * kNumBars;
             if (cnt[0]) { atomicAdd(&P.ctrl->n_active, (unsigned long long)cnt[0]); cnt[0] = 0; }
             if (cnt[1]) { atomicAdd(&P.ctrl->n_elists, (unsigned long long)cnt[1]); cnt[1] = 0; }
+            if (cnt[2]) { atomicAdd(&P.ctrl->n_quiet, (unsigned long long)cnt[2]); cnt[2] = 0; }
+            P.binact[blockIdx.x] = (int)cnt[3]; cnt[3] = 0;
         }
         if (threadIdx.x == 0) {
             P.pmax(cur ^ 1)[blockIdx.x] = rate;
@@ -325,7 +332,7 @@ namespace {
 static_assert(sizeof(HostEdge) == 24 && kDevPosMask == kPosMask && kDevKShift == kKShift && kDevSlotShift == kSlotShift &&
               kDevNoSlot == kNoSlot, "edge list encoding (mesh_builder.h / swe_kernels.cuh)");
 struct Layout {
-    size_t U0, U1, cellc, edges, tinfo, bvol, hint, zcell, perm, stage, pmax0, pmax1, qn, ctrl, gedges, cedge, eres, total;
+    size_t U0, U1, cellc, edges, tinfo, bvol, act0, act1, tnbr, binact, zcell, perm, stage, pmax0, pmax1, qn, ctrl, gedges, cedge, eres, total;
 };
 Layout make_layout(const HostTables &T, const TileTables &X, const GlobalEdges &E)
 {
@@ -335,7 +342,8 @@ Layout make_layout(const HostTables &T, const TileTables &X, const GlobalEdges &
     L.cellc = take(X.cellc.size() * sizeof(double)); L.edges = take(X.edges.size() * sizeof(HostEdge));
     L.tinfo = take(X.tinfo.size() * sizeof(int32_t));
     L.bvol = take(((size_t)X.nbedges + 1) * sizeof(double));
-    L.hint = take(((size_t)X.ntiles + 1) * sizeof(int32_t));
+    L.act0 = take(((size_t)X.ntiles + 1) * sizeof(int32_t)); L.act1 = take(((size_t)X.ntiles + 1) * sizeof(int32_t));
+    L.tnbr = take(X.tnbr.size() * sizeof(int32_t)); L.binact = take(kMaxPart * sizeof(int32_t));
     L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
     L.stage = take(3 * n * sizeof(double));
     L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
@@ -469,9 +477,9 @@ int swe_get_tile_info(const swe_mesh *m, int32_t *tile_cells, int64_t *ntiles, i
     return SWE_OK;
 }
 
-int swe_get_step_bytes(const swe_mesh *m, double active_tiles, double edge_lists, double *bytes)
+int swe_get_step_bytes(const swe_mesh *m, double active_tiles, double edge_lists, double quiet_tiles, double *bytes)
 {
-    if (!m || !bytes || !(active_tiles >= 0.0) || !(edge_lists >= 0.0)) return SWE_ERR_INVALID_ARG;
+    if (!m || !bytes || !(active_tiles >= 0.0) || !(edge_lists >= 0.0) || !(quiet_tiles >= 0.0)) return SWE_ERR_INVALID_ARG;
     const TileTables &X = m->X;
     const double nt = (double)m->T.nt, ntiles = (double)X.ntiles, TC = (double)X.tile_cells;
     if (m->edge_kernel) {
@@ -484,8 +492,10 @@ int swe_get_step_bytes(const swe_mesh *m, double active_tiles, double edge_lists
     double b = 0.0;
     b += 32.0 * nt;                                   // every cell's record read (TMA bulk copy) ...
     b += 32.0 * nt;                                   // ... and written (256-bit store)
-    b += 32.0 * (double)X.nhalo;                      // halo records, one 32-byte sector each
-    b += ntiles * (16.0 + 4.0 * (double)std::min(X.max_halo, X.tile_cells) + 8.0);  // header, halo ids, hint in and out
+    const double voting = std::max(0.0, ntiles - quiet_tiles);   // tiles that gather their halo and vote
+    b += 32.0 * (double)X.nhalo * voting / ntiles;    // halo records, one 32-byte sector each (mean list length)
+    b += voting * (16.0 + 4.0 * (double)std::min(X.max_halo, X.tile_cells));   // header, halo ids
+    b += ntiles * (4.0 + 4.0) + (ntiles - voting + active_tiles) * 4.0 * kNbrs;  // activity flag in and out, neighbour rows
     b += active_tiles * 24.0 * TC;                    // cell constants of the tiles that are not all dry
     b += edge_lists * 24.0 * (double)X.edges.size() / ntiles;   // edge lists fetched (mean list length)
     *bytes = b;
@@ -607,7 +617,8 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.cellc = (const double *)(m->ws + L.cellc); P.edges = (const double *)(m->ws + L.edges);
     P.tinfo = (const int32_t *)(m->ws + L.tinfo);
     P.bvol = (double *)(m->ws + L.bvol);
-    P.hint = (int32_t *)(m->ws + L.hint);
+    P.act0 = (int32_t *)(m->ws + L.act0); P.act1 = (int32_t *)(m->ws + L.act1);
+    P.tnbr = (const int32_t *)(m->ws + L.tnbr); P.binact = (int32_t *)(m->ws + L.binact);
     m->d_zcell = (double *)(m->ws + L.zcell); m->d_inv = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
@@ -632,6 +643,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
         pack_device_edges(X, dev_edges);
         CK(cudaMemcpyAsync(m->ws + L.edges, dev_edges.data(), dev_edges.size() * sizeof(double), cudaMemcpyHostToDevice, s));
         CK(cudaMemcpyAsync(m->ws + L.tinfo, X.tinfo.data(), X.tinfo.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
+        CK(cudaMemcpyAsync(m->ws + L.tnbr, X.tnbr.data(), X.tnbr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
         if (m->edge_kernel) {
             CK(cudaMemcpyAsync(m->ws + L.gedges, m->E.edges.data(), m->E.edges.size() * sizeof(HostEdge), cudaMemcpyHostToDevice, s));
             CK(cudaMemcpyAsync(m->ws + L.cedge, m->E.cedge.data(), m->E.cedge.size() * sizeof(int32_t), cudaMemcpyHostToDevice, s));
@@ -673,7 +685,10 @@ static int set_state_common(swe_mesh *m, const double *h, const double *hu, cons
     m->cur = 0;
     m->have_state = false; m->have_rates = false;
     Ctrl c{}; c.t[0] = t0; c.t[1] = t0; c.t_end = INFINITY; c.bad_cell = INT32_MAX;
-    CK(cudaMemsetAsync(m->P.hint, 1, (size_t)m->X.ntiles * sizeof(int32_t), m->stream));   // nothing known yet: every tile active (!= 0)
+    // nothing known yet: every tile counts as active in the previous step (!= 0), so none is quiet
+    CK(cudaMemsetAsync(m->P.act0, 1, (size_t)m->X.ntiles * sizeof(int32_t), m->stream));
+    CK(cudaMemsetAsync(m->P.act1, 1, (size_t)m->X.ntiles * sizeof(int32_t), m->stream));
+    CK(cudaMemsetAsync(m->P.binact, 0, kMaxPart * sizeof(int32_t), m->stream));
     if (m->X.nbedges > 0) CK(cudaMemsetAsync(m->P.bvol, 0, (size_t)m->X.nbedges * sizeof(double), m->stream));
     CK(cudaMemcpyAsync(m->P.ctrl, &c, sizeof(Ctrl), cudaMemcpyHostToDevice, m->stream));
     swe_pack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_inv, h, hu, hv, m->d_zcell);
@@ -1004,6 +1019,7 @@ int swe_get_stats(swe_mesh *m, swe_stats *s)
     s->n_dry = ndry; s->n_clamped = (int64_t)c.n_clamped; s->n_nonfinite = nbad;
     s->active_tile_steps = (int64_t)c.n_active;
     s->edge_list_fetches = (int64_t)c.n_elists;
+    s->quiet_tile_steps = (int64_t)c.n_quiet;
     return SWE_OK;
 }
 
