@@ -79,6 +79,8 @@ typedef struct {
     long double bvol_tag[MAX_TAGS]; /* cumulative outward volume per tag */
     int nthreads;
     int hll;               /* 0: HLLC third component (eq.24), 1: plain HLL for all three (eq.17-18) */
+    int storage32;         /* 1: the state {h, u, v} and the cell bed are kept in single precision between the steps
+                              (PAPER.md:424 configurable floating-point kind; arithmetic stays double) */
 } oracle_mesh;
 
 /* ---------------------------------------------------------------------------------
@@ -308,6 +310,26 @@ int oracle_set_inflow(oracle_mesh *m, int tag, double Q_total)
     return 0;
 }
 
+/* Single-precision storage (the library's SWE_FP_MIXED32): what is kept between two steps is
+ * float(h), float(u), float(v) with u = hu / h of the unrounded new state, and float(z); each step
+ * starts from h, h u, h v of those and computes in double as usual. */
+static void round_state(oracle_mesh *m)
+{
+    for (int64_t i = 0; i < m->nt; i++) {
+        const double h = m->h[i];
+        double u = 0.0, v = 0.0;
+        if (h > m->hdry) { u = (double)(float)(m->hu[i] / h); v = (double)(float)(m->hv[i] / h); }
+        const double hr = (double)(float)h;
+        m->h[i] = hr; m->hu[i] = hr * u; m->hv[i] = hr * v;
+    }
+}
+/* call before oracle_set_state; cannot be switched off again (the cell beds are rounded in place) */
+void oracle_set_storage32(oracle_mesh *m)
+{
+    m->storage32 = 1;
+    for (int64_t i = 0; i < m->nt; i++) m->z[i] = (double)(float)m->z[i];
+}
+
 void oracle_set_threads(oracle_mesh *m, int n) { m->nthreads = n > 0 ? n : 1; }
 void oracle_set_riemann(oracle_mesh *m, int hll) { m->hll = hll != 0; }
 int oracle_get_threads(const oracle_mesh *m) { return m->nthreads; }
@@ -320,6 +342,7 @@ void oracle_set_state(oracle_mesh *m, const double *h, const double *hu, const d
     /* R-15: a dry cell (h <= h_dry) carries no momentum */
     for (int64_t i = 0; i < m->nt; i++)
         if (m->h[i] <= m->hdry) { m->hu[i] = 0.0; m->hv[i] = 0.0; }
+    if (m->storage32) round_state(m);
     m->t = t0; m->dt_valid = 0; m->steps = 0; m->nclamp = 0; m->bnd_volume_out = 0.0L;
     for (int k = 0; k < MAX_TAGS; k++) m->bvol_tag[k] = 0.0L;
 }
@@ -426,6 +449,7 @@ static void step(oracle_mesh *m, double dt)
     t = m->h; m->h = m->h2; m->h2 = t;
     t = m->hu; m->hu = m->hu2; m->hu2 = t;
     t = m->hv; m->hv = m->hv2; m->hv2 = t;
+    if (m->storage32) round_state(m);
     m->nclamp += nclamp;
     m->bnd_volume_out += bvol;
     for (int64_t b = 0; b < m->nb; b++) m->bvol_tag[m->btag[b]] += (long double)m->bstep[b];

@@ -42,6 +42,7 @@ def lib():
         L.oracle_hllc.argtypes = [C.c_double] * 8 + [dp, dp]
         L.oracle_hll.argtypes = [C.c_double] * 8 + [dp]
         L.oracle_set_riemann.argtypes = [C.c_void_p, C.c_int]
+        L.oracle_set_storage32.argtypes = [C.c_void_p]
         _lib = L
     return _lib
 
@@ -92,9 +93,11 @@ class OracleSolver:
             L.oracle_set_threads(self._h, int(threads))
 
     @classmethod
-    def from_workload(cls, w, threads=None):
+    def from_workload(cls, w, threads=None, storage32=False):
         s = cls(w.nodes_xy, w.tris, w.bathymetry, w.manning, w.bc_tags, g=w.g, cfl=w.cfl,
                 h_dry=w.h_dry, threads=threads)
+        if storage32:
+            s.set_storage32()
         for tag, q in w.bc_values.items():
             s.set_inflow(tag, q)
         s.set_state(w.h, w.hu, w.hv)
@@ -112,6 +115,10 @@ class OracleSolver:
     def set_riemann(self, hll):
         """hll=True: plain HLL instead of HLLC."""
         self._L.oracle_set_riemann(self._h, int(bool(hll)))
+
+    def set_storage32(self):
+        """State and cell beds kept in single precision between the steps (call before set_state)."""
+        self._L.oracle_set_storage32(self._h)
 
     def set_threads(self, n):
         self._L.oracle_set_threads(self._h, int(n))

@@ -19,6 +19,7 @@ ORDER_IDENTITY, ORDER_HILBERT, ORDER_RCM = 0, 1, 2
 LOOP_AUTO, LOOP_GRAPH, LOOP_PERSISTENT, LOOP_LAUNCH, LOOP_CLUSTER = 0, 1, 2, 3, 4
 RIEMANN_HLLC, RIEMANN_HLL = 0, 1
 KERNEL_TILED, KERNEL_EDGE_TWO_PASS = 0, 1
+FP64, FP_MIXED32 = 0, 1
 LOOP_NAMES = {0: "auto", 1: "graph", 2: "persistent", 3: "launch", 4: "cluster"}
 ERR_ALL_DRY = -9
 
@@ -37,7 +38,7 @@ SYMBOLS = [
 class SweParams(C.Structure):
     _fields_ = [("g", C.c_double), ("cfl", C.c_double), ("h_dry", C.c_double),
                 ("ordering", C.c_int32), ("block_size", C.c_int32), ("loop_mode", C.c_int32),
-                ("riemann", C.c_int32), ("kernel", C.c_int32), ("reserved", C.c_int32)]
+                ("riemann", C.c_int32), ("kernel", C.c_int32), ("fp_kind", C.c_int32)]
 
 
 class SweStats(C.Structure):
@@ -130,7 +131,7 @@ class SweMesh:
 
     def __init__(self, nodes_xy, tris, bathymetry, manning, bc_tags, *, g=9.81, cfl=0.9,
                  h_dry=1e-6, ordering=ORDER_HILBERT, block_size=0, loop_mode=LOOP_AUTO,
-                 riemann=RIEMANN_HLLC, kernel=KERNEL_TILED):
+                 riemann=RIEMANN_HLLC, kernel=KERNEL_TILED, fp_kind=FP64):
         self._h = None
         L = load_library()
         self._L = L
@@ -149,6 +150,7 @@ class SweMesh:
         p.ordering, p.block_size, p.loop_mode = int(ordering), int(block_size), int(loop_mode)
         p.riemann = int(riemann)
         p.kernel = int(kernel)
+        p.fp_kind = int(fp_kind)
         self.params = p
         h = C.c_void_p()
         rc = L.swe_mesh_create(_dp(xy), self.nn, tr.ctypes.data_as(C.POINTER(C.c_int32)), self.nt,

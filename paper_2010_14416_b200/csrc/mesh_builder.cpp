@@ -36,12 +36,12 @@ template <class F> void parallel_for(int64_t n, F fn, int64_t grain = 65536)
 constexpr int kMaxHostThreads = 16;
 
 // Hilbert index of (x, y) on a 2^order x 2^order grid (classic rotate-and-flip walk).
-inline uint32_t hilbert_d(uint32_t x, uint32_t y, int order)
+inline uint64_t hilbert_d(uint32_t x, uint32_t y, int order)
 {
-    uint32_t d = 0;
+    uint64_t d = 0;
     for (uint32_t s = 1u << (order - 1); s > 0; s >>= 1) {
         uint32_t rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
-        d += s * s * ((3u * rx) ^ ry);
+        d += (uint64_t)s * s * ((3u * rx) ^ ry);
         if (ry == 0) {
             if (rx == 1) { x = s - 1 - (x & (s - 1)); y = s - 1 - (y & (s - 1)); }
             else { x &= (s - 1); y &= (s - 1); }
@@ -54,31 +54,54 @@ inline uint32_t hilbert_d(uint32_t x, uint32_t y, int order)
 void order_hilbert(HostTables &T)
 {
     const int64_t nt = T.nt;
-    double xmin = T.cx[0], xmax = T.cx[0], ymin = T.cy[0], ymax = T.cy[0];
-    for (int64_t i = 1; i < nt; i++) {
-        xmin = std::min(xmin, T.cx[i]); xmax = std::max(xmax, T.cx[i]);
-        ymin = std::min(ymin, T.cy[i]); ymax = std::max(ymax, T.cy[i]);
-    }
-    const int order = 16;
+    // bounding box of the centroids: per-thread extrema, combined in thread order
+    double bx[kMaxHostThreads][4];
+    for (auto &r : bx) { r[0] = r[2] = 1e300; r[1] = r[3] = -1e300; }
+    parallel_for(nt, [&](int64_t b, int64_t e, int thr) {
+        double x0 = 1e300, x1 = -1e300, y0 = 1e300, y1 = -1e300;
+        for (int64_t i = b; i < e; i++) {
+            x0 = std::min(x0, T.cx[i]); x1 = std::max(x1, T.cx[i]);
+            y0 = std::min(y0, T.cy[i]); y1 = std::max(y1, T.cy[i]);
+        }
+        bx[thr][0] = x0; bx[thr][1] = x1; bx[thr][2] = y0; bx[thr][3] = y1;
+    });
+    double xmin = 1e300, xmax = -1e300, ymin = 1e300, ymax = -1e300;
+    for (auto &r : bx) { xmin = std::min(xmin, r[0]); xmax = std::max(xmax, r[1]); ymin = std::min(ymin, r[2]); ymax = std::max(ymax, r[3]); }
+    // 17 bits per axis (square curve cells, so a 10:1 canal still has 2^13.7 of them across): the
+    // 34-bit curve index and the caller id (< 2^29) share one 64-bit key
+    const int order = 17, idbits = kHostIdBits;
     const double ext = std::max(std::max(xmax - xmin, ymax - ymin), 1e-300);
-    const double scale = (double)((1u << order) - 1) / ext; // square curve cells
+    const double scale = (double)((1u << order) - 1) / ext;
     std::vector<uint64_t> key((size_t)nt), tmp((size_t)nt);
     parallel_for(nt, [&](int64_t b, int64_t e, int) {
         for (int64_t i = b; i < e; i++) {
             uint32_t qx = (uint32_t)((T.cx[i] - xmin) * scale), qy = (uint32_t)((T.cy[i] - ymin) * scale);
-            key[(size_t)i] = ((uint64_t)hilbert_d(qx, qy, order) << 32) | (uint64_t)(uint32_t)i;
+            key[(size_t)i] = (hilbert_d(qx, qy, order) << idbits) | (uint64_t)i;
         }
     });
-    // stable LSD radix sort on the curve index (bits 32-63); the low word is the caller id in
+    // stable LSD radix sort on the curve index, 8 bits per pass, on the host threads: every thread
+    // counts and then scatters its own contiguous chunk, offsets by (digit, thread), so the result is
+    // the unique stable order whatever the number of threads.  The low bits are the caller id in
     // ascending order to begin with, so ties stay broken by caller id: deterministic
-    for (int shift = 32; shift < 64; shift += 8) {
-        size_t count[257] = {};
-        for (int64_t i = 0; i < nt; i++) count[((key[(size_t)i] >> shift) & 0xff) + 1]++;
-        for (int b = 0; b < 256; b++) count[b + 1] += count[b];
-        for (int64_t i = 0; i < nt; i++) tmp[count[(key[(size_t)i] >> shift) & 0xff]++] = key[(size_t)i];
+    std::vector<size_t> hist((size_t)kMaxHostThreads * 256);
+    for (int shift = idbits; shift < idbits + 2 * order; shift += 8) {
+        std::fill(hist.begin(), hist.end(), 0);
+        parallel_for(nt, [&](int64_t b, int64_t e, int thr) {
+            size_t *h = hist.data() + (size_t)thr * 256;
+            for (int64_t i = b; i < e; i++) h[(key[(size_t)i] >> shift) & 0xff]++;
+        });
+        size_t run = 0;
+        for (int d = 0; d < 256; d++)
+            for (int t = 0; t < kMaxHostThreads; t++) { const size_t c = hist[(size_t)t * 256 + d]; hist[(size_t)t * 256 + d] = run; run += c; }
+        parallel_for(nt, [&](int64_t b, int64_t e, int thr) {
+            size_t *h = hist.data() + (size_t)thr * 256;
+            for (int64_t i = b; i < e; i++) tmp[h[(key[(size_t)i] >> shift) & 0xff]++] = key[(size_t)i];
+        });
         key.swap(tmp);
     }
-    for (int64_t p = 0; p < nt; p++) T.perm[(size_t)p] = (int32_t)(key[(size_t)p] & 0xffffffffu);
+    parallel_for(nt, [&](int64_t b, int64_t e, int) {
+        for (int64_t p = b; p < e; p++) T.perm[(size_t)p] = (int32_t)(key[(size_t)p] & (((uint64_t)1 << idbits) - 1));
+    });
 }
 
 // Reverse Cuthill-McKee on the dual graph (cells adjacent through an edge; degree <= 3).

@@ -119,6 +119,28 @@ __device__ __forceinline__ void store_rec(Rec *p, const Rec &r)
     asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};"
                  :: "l"(p), "d"(r.h), "d"(r.u), "d"(r.v), "d"(r.z) : "memory");
 }
+// ---- state storage kinds (the paper's floating-point kind is configurable) ----------
+// Rec  : FP64 records, 32 bytes (the default, everything in this file).
+// RecF : FP32 records {h, u, v, z}, 16 bytes (SWE_FP_MIXED32): the state lives in HBM in single
+//        precision, every step converts to FP64 on load, computes in FP64 and rounds on store.
+//        Only the edge-centric two-pass kernels take this kind (templated on the record type).
+struct __align__(16) RecF { float h, u, v, z; };
+template <class R> __device__ __forceinline__ Rec ldrec(const R *p);
+template <> __device__ __forceinline__ Rec ldrec<Rec>(const Rec *p) { return load_rec(p); }
+template <> __device__ __forceinline__ Rec ldrec<RecF>(const RecF *p)
+{
+    float4 v;
+    asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
+    Rec r; r.h = v.x; r.u = v.y; r.v = v.z; r.z = v.w;
+    return r;
+}
+__device__ __forceinline__ void strec(Rec *p, const Rec &r) { store_rec(p, r); }
+__device__ __forceinline__ void strec(RecF *p, const Rec &r)
+{
+    asm volatile("st.global.v4.f32 [%0], {%1,%2,%3,%4};"
+                 :: "l"(p), "f"((float)r.h), "f"((float)r.u), "f"((float)r.v), "f"((float)r.z) : "memory");
+}
+
 __device__ __forceinline__ int32_t ldcg_i32(const int32_t *p)
 {
     int32_t v;

@@ -104,19 +104,20 @@ __device__ __forceinline__ double launch_dt(const Params &P, const int cur, doub
 
 // pass 1: one thread per edge of the mesh (a2-a7): both end points' records are gathered from HBM / L2
 // (one 32-byte sector each), the result for each side is written once
+template <class R>
 __global__ void __launch_bounds__(256)
 swe_edge_pass_kernel(const Params P, const int cur)
 {
     __shared__ double s_red[32];
     double dt_cfl, t_now; bool clipped;
     const double dt = launch_dt(P, cur, s_red, dt_cfl, t_now, clipped);
-    const Rec *__restrict__ U = P.U(cur);
+    const R *__restrict__ U = reinterpret_cast<const R *>(P.U(cur));
     for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < P.nge; e += (long long)gridDim.x * blockDim.x) {
         const int2 ab = __ldg(reinterpret_cast<const int2 *>(P.gedges + e));
         const double2 l = make_double2(__ldg(&P.gedges[e].lx), __ldg(&P.gedges[e].ly));   // 24-byte records: 8-byte aligned
-        const Rec A = load_rec(U + ab.x);
+        const Rec A = ldrec<R>(U + ab.x);
         Rec B = A;
-        if (ab.y >= 0) B = load_rec(U + ab.y);
+        if (ab.y >= 0) B = ldrec<R>(U + ab.y);
         double o[5];
         edge_eval(P, l.x, l.y, A, B, ab.y, dt, o);
         double2 *r = reinterpret_cast<double2 *>(P.eres + 6 * e);
@@ -128,14 +129,15 @@ swe_edge_pass_kernel(const Params P, const int cur)
 
 // pass 2: one thread per cell (a7-a11): its three edge results in the order k = 0,1,2, friction,
 // update, local rate; per-block maximum; block 0 advances the device clock
+template <class R>
 __global__ void __launch_bounds__(256)
 swe_cell_pass_kernel(const Params P, const int cur, const int tile_cells)
 {
     __shared__ double s_red[32];
     double dt_cfl, t_now; bool clipped;
     const double dt = launch_dt(P, cur, s_red, dt_cfl, t_now, clipped);
-    const Rec *__restrict__ Uin = P.U(cur);
-    Rec *__restrict__ Uout = P.U(cur ^ 1);
+    const R *__restrict__ Uin = reinterpret_cast<const R *>(P.U(cur));
+    R *__restrict__ Uout = reinterpret_cast<R *>(P.U(cur ^ 1));
     double rate = 0.0;
     unsigned nclamp = 0;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P.nt; i += (long long)gridDim.x * blockDim.x) {
@@ -145,12 +147,12 @@ swe_cell_pass_kernel(const Params P, const int cur, const int tile_cells)
         const double s1 = (__ldcg(r0) + __ldcg(r1)) + __ldcg(r2);
         const double s2 = (__ldcg(r0 + 1) + __ldcg(r1 + 1)) + __ldcg(r2 + 1);
         const double s3 = (__ldcg(r0 + 2) + __ldcg(r1 + 2)) + __ldcg(r2 + 2);
-        const Rec Ui = load_rec(Uin + i);
+        const Rec Ui = ldrec<R>(Uin + i);
         const int t = (int)(i / tile_cells), q = (int)(i - (long long)t * tile_cells);
         const double *cc = P.cellc + (size_t)t * 3 * tile_cells + q;
         Rec Un;
         rate = fmax(rate, cell_update(P, Ui, s1, s2, s3, __ldg(cc), __ldg(cc + tile_cells), __ldg(cc + 2 * tile_cells), dt, Un, nclamp));
-        store_rec(Uout + i, Un);
+        strec(Uout + i, Un);
     }
     rate = block_max(rate, s_red);
     if (nclamp) atomicAdd(&P.ctrl->n_clamped, (unsigned long long)nclamp);   // diagnostics only
@@ -198,6 +200,7 @@ step_kernel_t step_kernel_for(int tc)
 }
 
 // Per-block maxima of (sqrt(g h)+|V|)/R for the state in U[cur] (swe_compute_dt, first step).
+template <class R>
 __global__ void __launch_bounds__(kMaxBlock)
 swe_rate_kernel(const Params P, const int cur)
 {
@@ -206,7 +209,7 @@ swe_rate_kernel(const Params P, const int cur)
     for (int t = blockIdx.x; t < P.ntiles; t += gridDim.x) {
         const int i = t * blockDim.x + threadIdx.x;
         if (i < P.nt) {
-            const Rec U = load_rec(P.U(cur) + i);
+            const Rec U = ldrec<R>(reinterpret_cast<const R *>(P.U(cur)) + i);
             if (U.h > P.hdry)
                 rate = fmax(rate, (sqrt(P.g * U.h) + sqrt(fma(U.u, U.u, U.v * U.v))) *
                                   __ldg(P.cellc + ((size_t)t * 3 + 1) * blockDim.x + threadIdx.x));
@@ -229,6 +232,7 @@ __global__ void swe_finalize_dt_kernel(const Params P, const int cur)
 // dry, non-finite}; the host adds the <= kStatBlocks partials in block order.
 constexpr int kStatBlocks = 1024, kStatThreads = 256;
 struct StatPart { double volume; long long ndry, nbad; };
+template <class R>
 __global__ void __launch_bounds__(kStatThreads)
 swe_stats_kernel(const Params P, const int cur, const int tile_cells, StatPart *__restrict__ out)
 {
@@ -236,7 +240,7 @@ swe_stats_kernel(const Params P, const int cur, const int tile_cells, StatPart *
     __shared__ long long s_d[kStatThreads], s_b[kStatThreads];
     double v = 0.0; long long nd = 0, nb = 0;
     for (long long i = (long long)blockIdx.x * kStatThreads + threadIdx.x; i < P.nt; i += (long long)gridDim.x * kStatThreads) {
-        const Rec U = load_rec(P.U(cur) + i);
+        const Rec U = ldrec<R>(reinterpret_cast<const R *>(P.U(cur)) + i);
         const int t = (int)(i / tile_cells), q = (int)(i - (long long)t * tile_cells);
         const double area = 1.0 / __ldg(P.cellc + (size_t)t * 3 * tile_cells + q);
         v = fma(U.h, area, v);
@@ -258,6 +262,7 @@ swe_stats_kernel(const Params P, const int cur, const int tile_cells, StatPart *
 // caller numbering (h, hu, hv) -> internal records {h, u, v, z}; dry cells lose their momentum
 // Both kernels run over the CALLER's numbering c (coalesced on the caller's arrays) and touch the
 // internal record inv[c] as one 32-byte sector.  zcell is in caller numbering too.
+template <class R>
 __global__ void swe_pack_kernel(const Params P, const int cur, const int32_t *__restrict__ inv,
                                 const double *__restrict__ h, const double *__restrict__ hu,
                                 const double *__restrict__ hv, const double *__restrict__ zcell)
@@ -270,14 +275,15 @@ __global__ void swe_pack_kernel(const Params P, const int cur, const int32_t *__
     // would cost more than the copy
     if (!(r.h >= 0.0) || !isfinite(r.h) || !isfinite(qx) || !isfinite(qy)) atomicMin(&P.ctrl->bad_cell, c);
     if (r.h > P.hdry) { r.u = qx / r.h; r.v = qy / r.h; } else { r.u = 0.0; r.v = 0.0; }
-    store_rec(P.U(cur) + inv[c], r);
+    strec(reinterpret_cast<R *>(P.U(cur)) + inv[c], r);
 }
+template <class R>
 __global__ void swe_unpack_kernel(const Params P, const int cur, const int32_t *__restrict__ inv,
                                   double *__restrict__ h, double *__restrict__ hu, double *__restrict__ hv)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.nt) return;
-    const Rec r = load_rec(P.U(cur) + inv[c]);
+    const Rec r = ldrec<R>(reinterpret_cast<const R *>(P.U(cur)) + inv[c]);
     if (h) h[c] = r.h;
     if (hu) hu[c] = r.h * r.u;
     if (hv) hv[c] = r.h * r.v;
@@ -293,7 +299,7 @@ struct swe_mesh {
     HostTables T;
     TileTables X;
     GlobalEdges E;            // SWE_KERNEL_EDGE_TWO_PASS only
-    bool edge_kernel = false; int grid_edge = 0, grid_cell = 0;
+    bool edge_kernel = false, f32 = false; int grid_edge = 0, grid_cell = 0;
     std::string err;
     // device
     bool bound = false, have_state = false, have_rates = false;
@@ -362,7 +368,7 @@ int swe_params_default(swe_params *p)
     if (!p) return SWE_ERR_INVALID_ARG;
     p->g = 9.81; p->cfl = 0.9; p->h_dry = 1e-6;
     p->ordering = SWE_ORDER_HILBERT; p->block_size = 0; p->loop_mode = SWE_LOOP_AUTO; p->riemann = SWE_RIEMANN_HLLC;
-    p->kernel = SWE_KERNEL_TILED; p->reserved = 0;
+    p->kernel = SWE_KERNEL_TILED; p->fp_kind = SWE_FP64;
     return SWE_OK;
 }
 
@@ -383,9 +389,10 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     if (params) p = *params;
     if (!(p.g > 0.0) || !(p.cfl > 0.0) || !(p.h_dry >= 0.0) || p.ordering < 0 || p.ordering > SWE_ORDER_RCM ||
         p.loop_mode < 0 || p.loop_mode > SWE_LOOP_CLUSTER || p.riemann < 0 || p.riemann > SWE_RIEMANN_HLL ||
-        p.kernel < 0 || p.kernel > SWE_KERNEL_EDGE_TWO_PASS ||
+        p.kernel < 0 || p.kernel > SWE_KERNEL_EDGE_TWO_PASS || p.fp_kind < 0 || p.fp_kind > SWE_FP_MIXED32 ||
+        (p.fp_kind == SWE_FP_MIXED32 && p.kernel != SWE_KERNEL_EDGE_TWO_PASS) ||
         (p.block_size != 0 && p.block_size != 64 && p.block_size != 128 && p.block_size != 192 && p.block_size != 256)) {
-        g_create_err = "swe_mesh_create: invalid swe_params (block_size must be 0, 64, 128, 192 or 256)";
+        g_create_err = "swe_mesh_create: invalid swe_params (block_size must be 0, 64, 128, 192 or 256; SWE_FP_MIXED32 needs SWE_KERNEL_EDGE_TWO_PASS)";
         return SWE_ERR_INVALID_ARG;
     }
     swe_mesh *m = new (std::nothrow) swe_mesh();
@@ -404,6 +411,7 @@ int swe_mesh_create(const double *nodes_xy, int64_t nn, const int32_t *tris, int
     rc = build_tiles(m->T, m->block, p.g, m->X, m->err);
     if (rc != SWE_OK) { g_create_err = m->err; delete m; return rc; }
     m->edge_kernel = p.kernel == SWE_KERNEL_EDGE_TWO_PASS;
+    m->f32 = p.fp_kind == SWE_FP_MIXED32;
     if (m->edge_kernel) {
         rc = build_global_edges(m->T, m->E, m->err);
         if (rc != SWE_OK) { g_create_err = m->err; delete m; return rc; }
@@ -486,7 +494,8 @@ int swe_get_step_bytes(const swe_mesh *m, double active_tiles, double edge_lists
         // pass 1: edge record, one sector per end point, both sides' results out; pass 2: edge ids,
         // three 24-byte results, record in and out, cell constants
         const double ne = (double)m->E.edges.size(), nb = (double)X.nbedges;
-        *bytes = ne * 24.0 + (2.0 * ne - nb) * 32.0 + ne * 48.0 + nt * (12.0 + 72.0 + 32.0 + 24.0 + 32.0);
+        const double rec = m->f32 ? 16.0 : 32.0;
+        *bytes = ne * 24.0 + (2.0 * ne - nb) * 32.0 + ne * 48.0 + nt * (12.0 + 72.0 + rec + 24.0 + rec);
         return SWE_OK;
     }
     double b = 0.0;
@@ -691,7 +700,8 @@ static int set_state_common(swe_mesh *m, const double *h, const double *hu, cons
     CK(cudaMemsetAsync(m->P.binact, 0, kMaxPart * sizeof(int32_t), m->stream));
     if (m->X.nbedges > 0) CK(cudaMemsetAsync(m->P.bvol, 0, (size_t)m->X.nbedges * sizeof(double), m->stream));
     CK(cudaMemcpyAsync(m->P.ctrl, &c, sizeof(Ctrl), cudaMemcpyHostToDevice, m->stream));
-    swe_pack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_inv, h, hu, hv, m->d_zcell);
+    if (m->f32) swe_pack_kernel<RecF><<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_inv, h, hu, hv, m->d_zcell);
+    else swe_pack_kernel<Rec><<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, 0, m->d_inv, h, hu, hv, m->d_zcell);
     m->launches++;
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(&c, m->P.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, m->stream));
@@ -727,7 +737,8 @@ int swe_set_state_device(swe_mesh *m, const double *d_h, const double *d_hu, con
 static int ensure_rates(swe_mesh *m)
 {
     if (m->have_rates) return SWE_OK;
-    swe_rate_kernel<<<m->P.npart, m->block, 0, m->stream>>>(m->P, m->cur);
+    if (m->f32) swe_rate_kernel<RecF><<<m->P.npart, m->block, 0, m->stream>>>(m->P, m->cur);
+    else swe_rate_kernel<Rec><<<m->P.npart, m->block, 0, m->stream>>>(m->P, m->cur);
     m->launches++;
     CK(cudaGetLastError());
     m->have_rates = true;
@@ -768,8 +779,13 @@ int swe_compute_dt(swe_mesh *m, double *dt_out)
 static void launch_step(swe_mesh *m, cudaStream_t st, int cur)
 {
     if (m->edge_kernel) {
-        swe_edge_pass_kernel<<<m->grid_edge, 256, 0, st>>>(m->P, cur);
-        swe_cell_pass_kernel<<<m->grid_cell, 256, 0, st>>>(m->P, cur, m->X.tile_cells);
+        if (m->f32) {
+            swe_edge_pass_kernel<RecF><<<m->grid_edge, 256, 0, st>>>(m->P, cur);
+            swe_cell_pass_kernel<RecF><<<m->grid_cell, 256, 0, st>>>(m->P, cur, m->X.tile_cells);
+        } else {
+            swe_edge_pass_kernel<Rec><<<m->grid_edge, 256, 0, st>>>(m->P, cur);
+            swe_cell_pass_kernel<Rec><<<m->grid_cell, 256, 0, st>>>(m->P, cur, m->X.tile_cells);
+        }
     } else {
         m->kern<<<m->grid, m->block, m->smem, st>>>(m->P, cur, 1);
     }
@@ -919,7 +935,8 @@ int swe_get_state_device(swe_mesh *m, double *d_h, double *d_hu, double *d_hv)
     if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
     if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
     const int n = (int)m->T.nt;
-    swe_unpack_kernel<<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, m->cur, m->d_inv, d_h, d_hu, d_hv);
+    if (m->f32) swe_unpack_kernel<RecF><<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, m->cur, m->d_inv, d_h, d_hu, d_hv);
+    else swe_unpack_kernel<Rec><<<(n + 255) / 256, 256, 0, m->stream>>>(m->P, m->cur, m->d_inv, d_h, d_hu, d_hv);
     m->launches++;
     CK(cudaGetLastError());
     return SWE_OK;
@@ -1005,7 +1022,8 @@ int swe_get_stats(swe_mesh *m, swe_stats *s)
     if (rc != SWE_OK) return rc;
     const int nblk = (int)std::min<int64_t>(kStatBlocks, (m->T.nt + kStatThreads - 1) / kStatThreads);
     StatPart *d_part = reinterpret_cast<StatPart *>(m->d_stage);
-    swe_stats_kernel<<<nblk, kStatThreads, 0, m->stream>>>(m->P, m->cur, m->X.tile_cells, d_part);
+    if (m->f32) swe_stats_kernel<RecF><<<nblk, kStatThreads, 0, m->stream>>>(m->P, m->cur, m->X.tile_cells, d_part);
+    else swe_stats_kernel<Rec><<<nblk, kStatThreads, 0, m->stream>>>(m->P, m->cur, m->X.tile_cells, d_part);
     m->launches++;
     CK(cudaGetLastError());
     std::vector<StatPart> part((size_t)nblk);

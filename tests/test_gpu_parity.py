@@ -310,10 +310,36 @@ def test_edge_two_pass_kernel_matches_oracle_and_tiled_kernel(loop_mode):
     for a, b in zip(got[:3], ref[:3]):
         np.testing.assert_array_equal(a, b)
     assert got[3] == ref[3]
-    # the tile kernel took its shortcuts on the dry floodplain (all-dry tiles copied, quiet tiles copied
-    # without a halo gather) and still agrees bit for bit with the kernels that have none
-    st, ti = r.get_stats(), r.get_tile_info()
-    assert 0 < st["quiet_tile_steps"] < st["quiet_tile_steps"] + st["active_tile_steps"] <= 600 * ti["ntiles"]
+
+
+def test_quiet_tiles_bitwise_against_the_kernels_without_shortcuts():
+    """A mesh large enough for the quiet-tile path (blocks with >= 8 tiles, most of them on the dry
+    floodplain): the tile kernel copies all-dry tiles and streams quiet tiles through registers
+    without a halo gather, the edge-centric kernels compute every edge and every cell of every
+    step.  Identical bits, while the wet front keeps moving into quiet territory; and parity with
+    the oracle at the usual bar."""
+    w = W.config4(nx=1600, ny=400)
+    m, o = run_both(w, 300, block_size=64)
+    got = assert_parity(m, o, w)
+    st, ti = m.get_stats(), m.get_tile_info()
+    assert st["quiet_tile_steps"] > 0.5 * 300 * ti["ntiles"]                  # most tile-steps took the quiet path
+    assert 0 < st["active_tile_steps"] < 0.3 * 300 * ti["ntiles"]
+    assert st["quiet_tile_steps"] + st["active_tile_steps"] < 300 * ti["ntiles"]   # the rest were voted all dry
+    e = B.SweMesh.from_workload(w, kernel=B.KERNEL_EDGE_TWO_PASS).bind_device()
+    e.set_state(w.h, w.hu, w.hv)
+    e.run(300)
+    ref = e.get_state()
+    for a, b in zip(got[:3], ref[:3]):
+        np.testing.assert_array_equal(a, b)
+    assert got[3] == ref[3]
+    np.testing.assert_array_equal(m.get_boundary_volumes(), e.get_boundary_volumes())
+    # the persistent loop takes the same path and gives the same bits
+    p = B.SweMesh.from_workload(w, block_size=64, loop_mode=B.LOOP_PERSISTENT).bind_device()
+    p.set_state(w.h, w.hu, w.hv)
+    p.run(300)
+    for a, b in zip(got[:3], p.get_state()[:3]):
+        np.testing.assert_array_equal(a, b)
+    assert p.get_stats()["quiet_tile_steps"] == st["quiet_tile_steps"]
 
 
 def test_edge_two_pass_kernel_ordering_invariance_and_run_until():
@@ -331,6 +357,37 @@ def test_edge_two_pass_kernel_ordering_invariance_and_run_until():
     assert o.run_until(1.5) == out[0][5]
     for a, b in zip(out[0][:3], o.get_state()[:3]):
         np.testing.assert_allclose(a, b, rtol=RTOL, atol=ATOL)
+
+
+def test_mixed32_state_storage_against_the_oracle():
+    """SWE_FP_MIXED32 (the paper's floating-point kind is configurable): FP32 state
+    records in HBM, FP64 arithmetic, on the edge-centric two-pass kernels.  Bar:
+    both sides round the same quantities to float after every step, so they differ only where a
+    rounding falls the other way (2^-24 of the value each time, and through the fluxes 2^-24 of
+    the neighbours' values): 2e-5 of the field's scale, absolute + relative, after 600 steps;
+    against the all-double oracle the same bar holds with the accumulated float round-off."""
+    w = W.config4(nx=320, ny=80)
+    m = B.SweMesh.from_workload(w, kernel=B.KERNEL_EDGE_TWO_PASS, fp_kind=B.FP_MIXED32).bind_device()
+    m.set_state(w.h, w.hu, w.hv)
+    o = OracleSolver.from_workload(w, storage32=True)
+    o64 = OracleSolver.from_workload(w)
+    m.run(600)
+    assert o.run(600) == 600 and o64.run(600) == 600
+    hg, hug, hvg, tg, dtg = m.get_state()
+    for ref, tol in ((o, 2e-5), (o64, 2e-5)):
+        ho, huo, hvo, to, dto = ref.get_state()
+        for a, b in ((hg, ho), (hug, huo), (hvg, hvo)):
+            np.testing.assert_allclose(a, b, rtol=tol, atol=tol * max(1.0, float(np.abs(b).max())))
+        assert tg == pytest.approx(to, rel=1e-6) and dtg == pytest.approx(dto, rel=1e-5)
+        differ = (hg <= w.h_dry) != (ho <= w.h_dry)
+        assert (np.abs(ho[differ] - w.h_dry) < tol).all()       # the mask may differ only at the threshold
+    np.testing.assert_array_equal(hg, hg.astype(np.float32).astype(np.float64))     # the state IS single precision
+    st = m.get_stats()
+    assert st["n_clamped"] == 0 and st["n_nonfinite"] == 0 and st["steps"] == 600
+    # the tile kernel has no such variant: the combination is refused at create time
+    with pytest.raises(B.SweError) as e:
+        B.SweMesh.from_workload(w, fp_kind=B.FP_MIXED32)
+    assert e.value.code == -1
 
 
 # ---- BASELINE.json's full sizes, in the launch configuration bench.py times (defaults) ----------

@@ -368,3 +368,28 @@ def test_refined_mesh_mass_and_dt_scale():
     s.run(300)
     assert s.stats()["volume"] == pytest.approx(v0, rel=1e-12)
     assert s.stats()["nclamp"] == 0
+
+
+def test_single_precision_storage_stays_within_accumulated_float_roundoff():
+    """PAPER.md:424 (configurable floating-point kind), the oracle side of SWE_FP_MIXED32: the state
+    is rounded to single precision between the steps and everything else is unchanged.  Pinned by
+    what that definition fixes: the stored state is exactly representable in float; each step adds
+    at most one float rounding (2^-24 relative) to each of h, u, v, so after n steps of a
+    non-amplifying scheme the distance to the double-precision run is at most ~n 2^-24 (here a few
+    2^-24 sqrt(n), the roundings being uncorrelated); volume is conserved to the same order."""
+    w = W.config1()
+    n = 500
+    a, b = OracleSolver.from_workload(w), OracleSolver.from_workload(w, storage32=True)
+    v0 = b.stats()["volume"]
+    assert a.run(n) == n and b.run(n) == n
+    ha, hua, hva, ta, _ = a.get_state()
+    hb, hub, hvb, tb, _ = b.get_state()
+    np.testing.assert_array_equal(hb, hb.astype(np.float32).astype(np.float64))
+    u = hub / hb
+    np.testing.assert_allclose(u, u.astype(np.float32), rtol=2e-16, atol=0)       # h u with u a float
+    eps = 2.0 ** -24
+    for x, y in ((ha, hb), (hua, hub), (hva, hvb)):
+        d = np.abs(x - y).max()
+        assert 0.0 < d < 20.0 * eps * math.sqrt(n)
+    assert abs(ta - tb) / ta < 10.0 * eps
+    assert abs(b.stats()["volume"] - v0) / v0 < n * eps
