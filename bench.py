@@ -185,7 +185,8 @@ def job_throughput(cells_per_rank: int, steps: int, world: int, ms_max: float) -
 STATE_BYTES_DRY = 64.0        # an all-dry tile's update is the identity: its 32-byte records in and out
 
 
-def roofline_record(n, kernel_ms, active_share, list_share, step_bytes, tiles, peak, peak_src, quiet_share=None):
+def roofline_record(n, kernel_ms, active_share, list_share, step_bytes, tiles, peak, peak_src, quiet_share=None,
+                    kernel_name=None):
     """HBM roofline of one launch of the step kernel (= one time step of the whole mesh).
 
     frac cannot exceed ~1 for a correct kernel: it charges the SURVEY's 156 algorithmic bytes only
@@ -206,7 +207,7 @@ def roofline_record(n, kernel_ms, active_share, list_share, step_bytes, tiles, p
             "active_tile_share": active_share, "edge_list_share": list_share, "quiet_tile_share": quiet_share,
             "achieved_fixed_156": fixed / sec / 1e9, "frac_fixed_156": fixed / sec / 1e9 / peak,
             "frac_of_nominal_8TBs": algo / sec / 1e9 / 8000.0,
-            "kernel": f"swe_step_kernel<{tiles['tile_cells']}>", "peak_source": peak_src}
+            "kernel": kernel_name or f"swe_step_kernel<{tiles['tile_cells']}>", "peak_source": peak_src}
 
 
 def measure_device(B, w, args, dev, order, loop, barrier, world, sampler=None):
@@ -214,7 +215,8 @@ def measure_device(B, w, args, dev, order, loop, barrier, world, sampler=None):
     import torch
     n = w.ncells
     t_build = time.perf_counter()
-    m = B.SweMesh.from_workload(w, ordering=order, loop_mode=loop, block_size=args.block).bind_device(dev)
+    kern = {"tiled": B.KERNEL_TILED, "edge": B.KERNEL_EDGE_TWO_PASS}[args.kernel]
+    m = B.SweMesh.from_workload(w, ordering=order, loop_mode=loop, block_size=args.block, kernel=kern).bind_device(dev)
     t_build = time.perf_counter() - t_build
     m.set_state(w.h, w.hu, w.hv)
     m.run(args.warmup)
@@ -335,7 +337,8 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                    "mesh_build_s": round(r["t_build"], 2), "wet_fraction_end": 1.0 - stats["n_dry"] / n,
                    "n_clamped": stats["n_clamped"]},
         "roofline": roofline_record(n, kernel_ms, r["active_share"], r["list_share"], r["step_bytes"],
-                                    tiles, peak, peak_src, r["quiet_share"]),
+                                    tiles, peak, peak_src, r["quiet_share"],
+                                    "swe_edge_pass_kernel + swe_cell_pass_kernel" if args.kernel == "edge" else None),
         "cpu_baseline": {"value": cpu_value, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
                          "sample": what, "value_1_thread": getattr(time_oracle, "one_thread", None),
                          "host_cores": os.cpu_count()},
@@ -371,6 +374,8 @@ def main():
     ap.add_argument("--ordering", default="hilbert", choices=["hilbert", "rcm", "identity"])
     ap.add_argument("--loop", default="auto", choices=["auto", "graph", "persistent", "launch", "cluster"])
     ap.add_argument("--block", type=int, default=0, help="cells per tile = threads per block (0 = default)")
+    ap.add_argument("--kernel", default="tiled", choices=["tiled", "edge"],
+                    help="tiled = the fused tile kernel (default); edge = the edge-centric two-pass alternative (A/B only)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-wet", dest="wet", action="store_false",
                     help="skip the all-wet leg (config3) that the default run times beside the headline workload")

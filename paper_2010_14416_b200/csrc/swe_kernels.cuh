@@ -596,48 +596,47 @@ __device__ __forceinline__ int next_nonquiet(const unsigned *sq, int j, const in
     }
     return min(j, nmy);
 }
-__device__ __forceinline__ int next_quiet(const unsigned *sq, int j, const int nmy)
-{
-    const int lim = min(nmy, kMaxSeq);
-    while (j < lim) {
-        const unsigned w = sq[j >> 5] & (0xffffffffu << (j & 31));
-        if (w) { j = (j & ~31) + __ffs(w) - 1; return j < lim ? j : nmy; }
-        j = (j | 31) + 1;
-    }
-    return nmy;
-}
-// every quiet tile of the block's sequence: records from U(cur) to U(cur^1) through registers, four
+// every quiet tile of the block's sequence: records from U(cur) to U(cur^1) through registers, K
 // tiles in flight per thread; returns how many there were
 // (out of line, called once per step before the tile loop: its registers are its own)
+#ifndef SWE_QUIET_K
+#define SWE_QUIET_K 4
+#endif
 template <int TC>
 __device__ __noinline__ int copy_quiet_tiles(const int nt, const unsigned *sq, const Rec *__restrict__ Uin,
                                              Rec *__restrict__ Uout, int32_t *__restrict__ act_next, const int nmy)
 {
+    constexpr int K = SWE_QUIET_K;
     const int tid = threadIdx.x, G = gridDim.x;
-    int count = 0;
-    int j = next_quiet(sq, 0, nmy);
-    while (j < nmy) {
-        // (named variables, not arrays: the four records must stay in registers)
-        int t0 = -1, t1 = -1, t2 = -1, t3 = -1;
-        t0 = blockIdx.x + j * G; j = next_quiet(sq, j + 1, nmy); count++;
-        if (j < nmy) { t1 = blockIdx.x + j * G; j = next_quiet(sq, j + 1, nmy); count++; }
-        if (j < nmy) { t2 = blockIdx.x + j * G; j = next_quiet(sq, j + 1, nmy); count++; }
-        if (j < nmy) { t3 = blockIdx.x + j * G; j = next_quiet(sq, j + 1, nmy); count++; }
-        const long long i0 = (long long)t0 * TC + tid, i1 = (long long)t1 * TC + tid;
-        const long long i2 = (long long)t2 * TC + tid, i3 = (long long)t3 * TC + tid;
-        const bool p0 = i0 < nt, p1 = t1 >= 0 && i1 < nt, p2 = t2 >= 0 && i2 < nt, p3 = t3 >= 0 && i3 < nt;
+    const int lim = min(nmy, kMaxSeq), nwords = (lim + 31) >> 5;
+    int count = 0, wi = 0;
+    unsigned w = nwords > 0 ? sq[0] : 0u;            // the flag word being consumed lives in a register
+    for (;;) {
+        int t[K];
+#pragma unroll
+        for (int k = 0; k < K; k++) {
+            while (w == 0u && wi + 1 < nwords) w = sq[++wi];
+            t[k] = -1;
+            if (w) {
+                const int bit = __ffs(w) - 1;
+                w &= w - 1;
+                t[k] = blockIdx.x + ((wi << 5) + bit) * G;
+                count++;
+            }
+        }
+        if (t[0] < 0) break;
         // (unconditional loads from a valid address: a conditional one would put the record in local memory)
-        const Rec r0 = load_rec(Uin + (p0 ? i0 : 0)), r1 = load_rec(Uin + (p1 ? i1 : 0));
-        const Rec r2 = load_rec(Uin + (p2 ? i2 : 0)), r3 = load_rec(Uin + (p3 ? i3 : 0));
-        if (p0) store_rec(Uout + i0, r0);
-        if (p1) store_rec(Uout + i1, r1);
-        if (p2) store_rec(Uout + i2, r2);
-        if (p3) store_rec(Uout + i3, r3);
-        if (tid == 0) {
-            act_next[t0] = 0;
-            if (t1 >= 0) act_next[t1] = 0;
-            if (t2 >= 0) act_next[t2] = 0;
-            if (t3 >= 0) act_next[t3] = 0;
+        Rec r[K];
+#pragma unroll
+        for (int k = 0; k < K; k++) {
+            const long long i = (long long)t[k] * TC + tid;
+            r[k] = load_rec(Uin + (t[k] >= 0 && i < nt ? i : 0));
+        }
+#pragma unroll
+        for (int k = 0; k < K; k++) {
+            const long long i = (long long)t[k] * TC + tid;
+            if (t[k] >= 0 && i < nt) store_rec(Uout + i, r[k]);
+            if (t[k] >= 0 && tid == 0) act_next[t[k]] = 0;
         }
     }
     return count;
