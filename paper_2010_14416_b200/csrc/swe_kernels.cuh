@@ -11,7 +11,9 @@
 //            halo id and the activity hint a thread needs travel in its registers, loaded two
 //            tiles ahead.  A tile whose cells and halo are all dry (and that has no inflow edge)
 //            copies its records and skips everything else; the edge list of a tile that was
-//            like that at the previous step is not even requested.
+//            like that at the previous step is not even requested; and a tile that was like
+//            that together with all its neighbour tiles ("quiet") never enters the pipeline:
+//            its records stream from U(cur) to U(cur^1) through registers.
 //   phase 1  (edge-parallel) every edge that touches the tile is evaluated ONCE: hydrostatic
 //            reconstruction, rotation, HLLC flux, rotation back, both sides' bathymetry source;
 //            the signed, length-weighted result goes to the (cell, local edge) slots of its end
@@ -505,9 +507,11 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 //   double  so2 [3][TC + 1]        entry per k staggers the banks of a cell's three slots
 //   double  scell[3][TC]           1/|Omega|, 1/R, g m^2
 //   uint64  bar[5]                 rec[2], edge[2], cell constants
+//   uint32  count[4], sq[128]      the producer thread's counters; quiet flags of the block's tiles
 //   Rec     srec[2][TC + MH]       state records of the tile's cells, then of its halo cells
 //   uint2 + double2  sedge[2][ME]  the tile's edge list (24 bytes per edge)
-// Schedule for the block's n-th tile (s = n & 1), all copies asynchronous and one tile ahead:
+// Schedule for the block's n-th pipeline stage, i.e. its n-th tile that is not quiet (s = n & 1), all
+// copies asynchronous and one stage ahead:
 //   top      wait: own halo gathers, records of tile n; barrier (= the dry vote)
 //            issue: records of tile n+1 (bulk) -> srec[s^1]; edge list of tile n+1 (bulk) ->
 //                   sedge[s^1] if that tile was active a step ago; cell constants of tile n
