@@ -337,6 +337,7 @@ static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 namespace {
 static_assert(sizeof(HostEdge) == 24 && kDevPosMask == kPosMask && kDevKShift == kKShift && kDevSlotShift == kSlotShift &&
               kDevNoSlot == kNoSlot, "edge list encoding (mesh_builder.h / swe_kernels.cuh)");
+static_assert(kTileNbrs == kNbrs && sizeof(HostEdge) == sizeof(GEdge), "neighbour-tile rows / global edge records");
 struct Layout {
     size_t U0, U1, cellc, edges, tinfo, bvol, act0, act1, tnbr, binact, zcell, perm, stage, pmax0, pmax1, qn, ctrl, gedges, cedge, eres, total;
 };
