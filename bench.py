@@ -190,12 +190,15 @@ def roofline_record(n, kernel_ms, active_share, list_share, step_bytes, tiles, p
     """HBM roofline of one launch of the step kernel (= one time step of the whole mesh).
 
     frac cannot exceed ~1 for a correct kernel: it charges the SURVEY's 156 algorithmic bytes only
-    to the cells of tiles that did the method's work in the timed steps and 64 bytes (record in and
-    out) to the cells of all-dry tiles, whose update is the identity (counted on the device).
+    to the cells of tiles that did the method's work in the timed steps, 64 bytes (record in and
+    out) to the cells of all-dry tiles that were moved, whose update is the identity, and nothing to
+    the cells of quiet tiles, whose records are in place in both state buffers and are not touched
+    (all three counted on the device).
     traffic = the bytes this launch requested from memory according to the library's own table
     sizes and the same counters (swe_get_step_bytes), not a stored constant."""
     sec = kernel_ms * 1e-3
-    algo = (ALGO_BYTES_PER_CELL * active_share + STATE_BYTES_DRY * (1.0 - active_share)) * n
+    qs = quiet_share or 0.0
+    algo = (ALGO_BYTES_PER_CELL * active_share + STATE_BYTES_DRY * max(0.0, 1.0 - active_share - qs)) * n
     fixed = ALGO_BYTES_PER_CELL * n
     return {"bound": "hbm", "achieved": algo / sec / 1e9, "peak": peak, "unit": "GB/s",
             "frac": algo / sec / 1e9 / peak, "traffic": step_bytes,
@@ -203,7 +206,7 @@ def roofline_record(n, kernel_ms, active_share, list_share, step_bytes, tiles, p
                             "device counters (swe_get_step_bytes); ncu dram__bytes cross-check in profiles/",
             "achieved_traffic": step_bytes / sec / 1e9, "frac_traffic": step_bytes / sec / 1e9 / peak,
             "algorithmic_bytes_per_launch": algo, "algorithmic_bytes_per_cell_active_tile": ALGO_BYTES_PER_CELL,
-            "algorithmic_bytes_per_cell_dry_tile": STATE_BYTES_DRY,
+            "algorithmic_bytes_per_cell_dry_tile": STATE_BYTES_DRY, "algorithmic_bytes_per_cell_quiet_tile": 0.0,
             "active_tile_share": active_share, "edge_list_share": list_share, "quiet_tile_share": quiet_share,
             "achieved_fixed_156": fixed / sec / 1e9, "frac_fixed_156": fixed / sec / 1e9 / peak,
             "frac_of_nominal_8TBs": algo / sec / 1e9 / 8000.0,

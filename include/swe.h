@@ -115,8 +115,8 @@ typedef struct {
                                   a tile that was all dry at the previous step is read only if the tile turns
                                   out active): with active_tile_steps it fixes the bytes a step requests */
     int64_t quiet_tile_steps;  /* sum over the steps of the number of QUIET tiles: inactive in the previous step with
-                                  all their neighbour tiles, hence all dry now; their records are copied through
-                                  registers without a halo gather or a vote */
+                                  all their neighbour tiles, hence all dry now, and with their records already in
+                                  place in both state buffers: they are not touched */
 } swe_stats;
 
 /* Fills *p with the defaults listed above. */
@@ -271,9 +271,9 @@ int swe_get_tile_info(const swe_mesh *mesh, int32_t *tile_cells, int64_t *ntiles
 /*
  * Bytes one time step REQUESTS from device memory, from the library's own table sizes, given how
  * many tiles are active (not all dry), how many tile edge lists are fetched and how many tiles are
- * quiet (copied without a halo gather) in that step (per-step averages taken from swe_stats.
- * active_tile_steps / edge_list_fetches / quiet_tile_steps): every cell's 32-byte record in and
- * out, one 32-byte sector per halo record of a tile that is not quiet, tile headers + halo ids,
+ * quiet (not touched) in that step (per-step averages taken from swe_stats.
+ * active_tile_steps / edge_list_fetches / quiet_tile_steps): the 32-byte record in and out of every
+ * cell of a tile that is not quiet, one 32-byte sector per halo record of such a tile, tile headers + halo ids,
  * activity flags and neighbour-tile rows,
  * 24 bytes of cell constants per cell of an active tile, 24 bytes per edge of a fetched list (mean
  * list length).  This is the kernel's request stream, not a DRAM counter: L2 hits on the halo

@@ -12,8 +12,10 @@
 //            tiles ahead.  A tile whose cells and halo are all dry (and that has no inflow edge)
 //            copies its records and skips everything else; the edge list of a tile that was
 //            like that at the previous step is not even requested; and a tile that was like
-//            that together with all its neighbour tiles ("quiet") never enters the pipeline:
-//            its records stream from U(cur) to U(cur^1) through registers.
+//            that together with all its neighbour tiles ("quiet") never enters the pipeline and
+//            is not touched at all: the previous step copied its records unchanged, so both state
+//            buffers hold them already.  A block that runs out of tiles takes some from the
+//            lists of others ("work stealing").
 //   phase 1  (edge-parallel) every edge that touches the tile is evaluated ONCE: hydrostatic
 //            reconstruction, rotation, HLLC flux, rotation back, both sides' bathymetry source;
 //            the signed, length-weighted result goes to the (cell, local edge) slots of its end
@@ -76,7 +78,7 @@ struct Ctrl {                 // device-resident loop state
     unsigned long long n_clamped;
     unsigned long long n_active;  // tiles that were not all dry, summed over the steps (diagnostics)
     unsigned long long n_elists;  // edge lists fetched, summed over the steps (diagnostics)
-    unsigned long long n_quiet;   // quiet tiles (copied through registers), summed over the steps (diagnostics)
+    unsigned long long n_quiet;   // quiet tiles (left untouched), summed over the steps (diagnostics)
     int all_dry;              // set when a step found no wet cell
     int bad_cell;             // smallest caller id with a negative depth or a non-finite value (swe_set_state)
 };
@@ -90,7 +92,10 @@ struct Params {
     double *bvol;             // [boundary edges] cumulative outward volume through each boundary edge
     int32_t *act0, *act1;     // [ntiles] 1 if the tile was active (not all dry) in the step that produced U0 / U1
     const int32_t *tnbr;      // [ntiles][kNbrs] tiles owning each tile's halo cells (-1 padding; [0] = -2: never quiet)
-    int32_t *binact;          // [npart] inactive tiles of each block's sequence in the previous step
+    int32_t *binact;          // [npart] inactive tiles each block walked through in the previous step
+    unsigned long long *wq;   // [npart] work word of each block's tile list: head / tail claims, see "work stealing"
+    int32_t *wlist;           // [npart][wstride] tiles of each block's list that are not quiet (published when quiet tiles were looked for)
+    int32_t wstride;          // = ceil(ntiles / npart)
     double *pmax0, *pmax1;    // [npart] per-block max rate of state U0 / U1
     Ctrl *ctrl;
     // edge-centric two-pass kernels only (SWE_KERNEL_EDGE_TWO_PASS; NULL otherwise)
@@ -507,7 +512,9 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 //   double  so2 [3][TC + 1]        entry per k staggers the banks of a cell's three slots
 //   double  scell[3][TC]           1/|Omega|, 1/R, g m^2
 //   uint64  bar[5]                 rec[2], edge[2], cell constants
-//   uint32  count[4], sq[128]      the producer thread's counters; quiet flags of the block's tiles
+//   uint32  count[4]               the producer thread's counters
+//   int32   ring[4], claim[4]      tiles of the coming pipeline stages; the producer thread's claim state
+//   uint32  sq[128]                quiet flags of the block's tiles
 //   Rec     srec[2][TC + MH]       state records of the tile's cells, then of its halo cells
 //   uint2 + double2  sedge[2][ME]  the tile's edge list (24 bytes per edge)
 // Schedule for the block's n-th pipeline stage, i.e. its n-th tile that is not quiet (s = n & 1), all
@@ -531,7 +538,8 @@ template <int TC> struct SmemLayout {
     static constexpr int so2 = so01 + 3 * PLC * 16;
     static constexpr int scell = (so2 + 3 * PLC * 8 + 15) & ~15;
     static constexpr int bar = scell + 3 * TC * 8;
-    static constexpr int sq = bar + kNumBars * 8 + 16;                   // after four diagnostic counters
+    static constexpr int ring = bar + kNumBars * 8 + 16;                 // after four diagnostic counters
+    static constexpr int sq = ring + 32;                                 // after the ring and the claim state
     static constexpr int srec = (sq + kMaxSeq / 8 + 31) & ~31;
 };
 __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int ME)
@@ -540,7 +548,7 @@ __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int M
     size_t o = 3 * PLC * 16;
     o = (o + 3 * PLC * 8 + 15) & ~(size_t)15;
     o += 3 * (size_t)TC * 8;
-    o = (o + kNumBars * 8 + 16 + 4096 / 8 + 31) & ~(size_t)31;           // barriers, counters, quiet flags (kMaxSeq bits)
+    o = (o + kNumBars * 8 + 16 + 32 + 4096 / 8 + 31) & ~(size_t)31;      // barriers, counters, ring + claim state, quiet flags (kMaxSeq bits)
     o += 2 * (size_t)(TC + MH) * sizeof(Rec);
     o += 2 * (size_t)ME * 24;
     return o;
@@ -556,9 +564,12 @@ struct PipeState { unsigned n = 0, epar = 0, cpar = 0; };
 // tile that was inactive in the previous step, and whose halo cells all belong to tiles that were
 // inactive in the previous step too, is QUIET: none of its cells and none of its halo cells has
 // changed since they were seen dry, so it is all dry now, and its update is the identity whatever
-// its neighbours do in this step.  A quiet tile needs no halo gather, no vote, no shared memory: its
-// records go from U(cur) to U(cur^1) through registers, four tiles in flight per thread, which is
-// what keeps HBM busy on the dry part of a mesh (the paper's river domains are mostly dry land).
+// its neighbours do in this step.  And the identity is already in place: the previous step, in which
+// the tile was inactive, wrote U(cur)[tile] = U(cur^1)[tile] bit for bit, and nothing has written
+// U(cur^1)[tile] since, so the buffer this step writes holds the tile's records already.  A quiet
+// tile therefore costs one flag (act(cur^1)[t] = 0) and no traffic on the state: no halo gather, no
+// vote, no copy -- the paper's river domains are mostly dry land, and that part
+// of the mesh now costs nothing per step.
 // Tiles with an inflow edge or with more than kTileNbrs neighbour tiles are never quiet (tnbr[0] = -2).
 // The block's tiles are tile(j) = blockIdx.x + j gridDim.x; bit j of sq[] says tile(j) is quiet.
 
@@ -600,57 +611,100 @@ __device__ __forceinline__ int next_nonquiet(const unsigned *sq, int j, const in
     }
     return min(j, nmy);
 }
-// every quiet tile of the block's sequence: records from U(cur) to U(cur^1) through registers, K
-// tiles in flight per thread; returns how many there were
-// (out of line, called once per step before the tile loop: its registers are its own)
-#ifndef SWE_QUIET_K
-#define SWE_QUIET_K 4
+// ---- work stealing ---------------------------------------------------------------------------------
+// Block b OWNS the tiles tile(j) = b + j gridDim.x; the ones that are not quiet form its list, in the order
+// of j.  The blocks of an SM do not advance at the same pace (the warp schedulers favour some warp
+// slots: measured, the four blocks of an SM finished their equal shares 115 to 155 us after the launch),
+// and the wet part of a mesh is not spread evenly, so a block that has emptied its list takes tiles
+// from the lists of others.  P.wq[b] is the list's work word: bits 0-30 head = entries the owner has
+// claimed from the front (atomicAdd 1), bit 31 set if the list is spelled out in P.wlist (quiet tiles
+// were looked for; otherwise entry k is tile b + k gridDim.x), bits 32-63 tail (signed) = end of the
+// unclaimed part, which a thief lowers (atomicAdd -2^32) to claim entry tail - 1.  Either claim is good
+// iff head < tail in the word the atomic returned; both counters move one way only, so no entry is given
+// out twice, and the owner goes on until a claim of its own fails, so every word ends a step exhausted
+// (head >= tail) and a thief that reads a word its owner has not yet set up for this step finds nothing.
+// The results do not depend on which block computes a tile (per-cell arithmetic, maxima, single-writer
+// boundary accumulators), so they are the same bits with or without stealing.
+// All of it is done by the block's producer thread while its warp waits for the longer edge loops of
+// the first warps; the tile of the stage after the next one goes to the others through a ring.
+struct ClaimState {
+    int src;       // list being consumed: own block first, then victims; -1: nothing left anywhere
+    int jc;        // own list: next position of the block's sequence to look at
+    int pre;       // own claims already contained in the initial work word
+    int fails;     // probe rounds that found no victim since the last good claim
+};
+constexpr unsigned long long kTailOne = 1ull << 32;
+constexpr unsigned kListBit = 0x80000000u;
+#ifndef SWE_PROBE_ROUNDS
+#define SWE_PROBE_ROUNDS 2
 #endif
-template <int TC>
-__device__ __noinline__ int copy_quiet_tiles(const int nt, const unsigned *sq, const Rec *__restrict__ Uin,
-                                             Rec *__restrict__ Uout, int32_t *__restrict__ act_next, const int nmy)
-{
-    constexpr int K = SWE_QUIET_K;
-    const int tid = threadIdx.x, G = gridDim.x;
-    const int lim = min(nmy, kMaxSeq), nwords = (lim + 31) >> 5;
-    int count = 0, wi = 0;
-    unsigned w = nwords > 0 ? sq[0] : 0u;            // the flag word being consumed lives in a register
-    for (;;) {
-        int t[K];
-#pragma unroll
-        for (int k = 0; k < K; k++) {
-            while (w == 0u && wi + 1 < nwords) w = sq[++wi];
-            t[k] = -1;
-            if (w) {
-                const int bit = __ffs(w) - 1;
-                w &= w - 1;
-                t[k] = blockIdx.x + ((wi << 5) + bit) * G;
-                count++;
+constexpr int kProbe = 8, kProbeRounds = SWE_PROBE_ROUNDS;
+
+template <bool QUIET>
+__device__ __noinline__ int claim_tile(unsigned long long *const wq, const int32_t *const wlist, const int wstride,
+                                       ClaimState *cs, const unsigned *sq, const int nmy)
+{   // (the kernel parameters by value: a reference would put the whole parameter block on the stack)
+    const int b = blockIdx.x, G = gridDim.x;
+    if (cs->src == b) {
+        const int j = QUIET ? next_nonquiet(sq, cs->jc, nmy) : min(cs->jc, nmy);
+        if (j < nmy) {
+            cs->jc = j + 1;
+            bool ok = true;
+            if (cs->pre > 0) cs->pre--;
+            else {
+                const unsigned long long old = atomicAdd(wq + b, 1ull);
+                ok = (int)((unsigned)old & ~kListBit) < (int)(unsigned)(old >> 32);
             }
+            if (ok) return b + j * G;
         }
-        if (t[0] < 0) break;
-        // (unconditional loads from a valid address: a conditional one would put the record in local memory)
-        Rec r[K];
-#pragma unroll
-        for (int k = 0; k < K; k++) {
-            const long long i = (long long)t[k] * TC + tid;
-            r[k] = load_rec(Uin + (t[k] >= 0 && i < nt ? i : 0));
-        }
-#pragma unroll
-        for (int k = 0; k < K; k++) {
-            const long long i = (long long)t[k] * TC + tid;
-            if (t[k] >= 0 && i < nt) store_rec(Uout + i, r[k]);
-            if (t[k] >= 0 && tid == 0) act_next[t[k]] = 0;
-        }
+        cs->src = -2;                       // own list finished, or the rest of it was taken: look for a victim
     }
-    return count;
+    if (cs->src == -1) return -1;
+    for (;;) {
+        if (cs->src >= 0) {
+            const int v = cs->src;
+            const unsigned long long old = atomicAdd(wq + v, 0ull - kTailOne);
+            const int h = (int)((unsigned)old & ~kListBit), t = (int)(unsigned)(old >> 32);
+            if (h < t) {
+                cs->fails = 0;
+                if (!((unsigned)old & kListBit)) return v + (t - 1) * G;
+                __threadfence();            // the list was published before the word
+                return ldcg_i32(wlist + (size_t)v * wstride + (t - 1));
+            }
+            cs->src = -2;
+        }
+        if (cs->fails >= kProbeRounds) { cs->src = -1; return -1; }
+        // a handful of candidates per round: the blocks that share this block's SM when blocks are dealt
+        // round-robin (b + G/4, ...), its neighbours, a few scattered ones; the one furthest behind wins
+        int best = -1, best_rem = 0;
+        const unsigned salt = (unsigned)b * 2654435761u + (unsigned)cs->fails * 40503u + (unsigned)cs->jc * 9973u;
+        int cand[kProbe];
+        unsigned long long w[kProbe];
+#pragma unroll
+        for (int q = 0; q < kProbe; q++) {
+            int v;
+            if (cs->fails == 0 && q < 3) v = b + (q + 1) * (G >> 2);
+            else if (cs->fails == 0 && q < 5) v = b + (q == 3 ? 1 : G - 1);
+            else v = (int)((salt + (unsigned)q * 2246822519u) >> 8);
+            cand[q] = (int)((unsigned)v % (unsigned)G);
+            asm volatile("ld.global.cg.u64 %0, [%1];" : "=l"(w[q]) : "l"(wq + cand[q]) : "memory");
+        }
+#pragma unroll
+        for (int q = 0; q < kProbe; q++) {
+            const int rem = (int)(unsigned)(w[q] >> 32) - (int)((unsigned)w[q] & ~kListBit);
+            if (cand[q] != b && rem > best_rem) { best_rem = rem; best = cand[q]; }
+        }
+        cs->jc++;                           // (free once the own list is done: varies the scattered candidates)
+        if (best < 0) cs->fails++;
+        else cs->src = best;
+    }
 }
 
 // All the tiles of this block for one time step.
 // Returns this thread's maximum rate contribution.
-// QUIET: look for quiet tiles and copy them through registers first (chosen per block and step when
-// a good share of the block's tiles was inactive in the previous step; the results are the same
-// either way, an all-dry tile that is not treated as quiet is found by the vote).
+// QUIET: look for quiet tiles first and leave them alone (chosen per block and step when a good
+// share of the block's tiles was inactive in the previous step; the results are the same either way,
+// an all-dry tile that is not treated as quiet is found by the vote and copied).
 template <int TC, bool QUIET>
 __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *smem, const int cur,
                                              const double dt, unsigned &nclamp, PipeState &ps)
@@ -721,33 +775,65 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
     auto load_hid = [&](int t) { return tid < P.max_halo ? __ldg(P.tinfo + (size_t)t * istride + kInfoHdr + tid) : -1; };
     auto tile_of = [&](int j) { return (int)blockIdx.x + j * G; };
 
-    // ---- which of this block's tiles are quiet; the pipeline below runs over the others
-    auto next_stage = [&](int j) { if constexpr (QUIET) return next_nonquiet(sq, j, nmy); else return min(j, nmy); };
+    // ---- this block's list: the tiles of its sequence that are not quiet
+    int *const sring = reinterpret_cast<int *>(smem + SL::ring);
+    ClaimState *const cs = reinterpret_cast<ClaimState *>(smem + SL::ring + 16);
+    int len = nmy;
     if constexpr (QUIET) {
         quiet_flags<TC>(P, act_prev, sq, nmy);
         __syncthreads();
-        const int nq = copy_quiet_tiles<TC>(P.nt, sq, Uin, Uout, act_next, nmy);
-        if (producer) { scount[2] += (unsigned)nq; scount[3] += (unsigned)nq; }
+        // spell the list out for thieves: entry k = the k-th tile of the sequence that is not quiet
+        const int lim = min(nmy, kMaxSeq);
+        int32_t *const wl = P.wlist + (size_t)blockIdx.x * P.wstride;
+        int nq_all = 0;
+        for (int w = 0; w < (lim + 31) >> 5; w++) nq_all += __popc(sq[w]);
+        len = nmy - nq_all;
+        for (int j = tid; j < nmy; j += TC) {
+            int nq = nq_all;
+            bool quiet = false;
+            if (j < lim) {
+                nq = 0;
+                for (int w = 0; w < (j >> 5); w++) nq += __popc(sq[w]);
+                const unsigned word = sq[j >> 5];
+                nq += __popc(word & ((1u << (j & 31)) - 1u));
+                quiet = (word >> (j & 31)) & 1u;
+            }
+            if (!quiet) wl[j - nq] = (int)blockIdx.x + j * G;
+            else act_next[(int)blockIdx.x + j * G] = 0;    // all a quiet tile costs: its records are in place already
+        }
+        if (producer) { scount[2] += (unsigned)nq_all; scount[3] += (unsigned)nq_all; }
+        __threadfence();
+        __syncthreads();
     }
-    int j0 = next_stage(0);                              // this pipeline stage, the next one, the one after
-    int j1 = j0 < nmy ? next_stage(j0 + 1) : nmy;
-    if (j0 >= nmy) return 0.0;                           // nothing but quiet tiles
-    // ---- prologue: everything tile(j0) needs; header, halo id and hint of tile(j1)
-    int4 hdr0 = load_hdr(tile_of(j0)), hdr1 = make_int4(0, 0, 0, 0);
-    int hid0 = load_hid(tile_of(j0)), hid1 = -1, hint1 = 0;
+    if (producer) {
+        const int pre = min(len, 2);
+        P.wq[blockIdx.x] = ((unsigned long long)(unsigned)len << 32) | (QUIET ? kListBit : 0u) | (unsigned)pre;
+        cs->src = blockIdx.x; cs->jc = 0; cs->pre = pre; cs->fails = 0;
+    }
+    // the first two stages (a block with a shorter list of its own takes from others right away)
+    if (producer) {
+        sring[0] = claim_tile<QUIET>(P.wq, P.wlist, P.wstride, cs, sq, nmy);
+        sring[1] = claim_tile<QUIET>(P.wq, P.wlist, P.wstride, cs, sq, nmy);
+    }
+    __syncthreads();
+    int tile0 = sring[0], tile1 = sring[1];              // this pipeline stage, the next one
+    if (tile0 < 0) return 0.0;                           // nothing but quiet tiles here and nothing to take elsewhere
+    // ---- prologue: everything tile0 needs; header, halo id and hint of tile1
+    int4 hdr0 = load_hdr(tile0), hdr1 = make_int4(0, 0, 0, 0);
+    int hid0 = load_hid(tile0), hid1 = -1, hint1 = 0;
     bool req0 = true;                    // was this tile's edge list requested?  The step's first pipeline stage: always
     if (producer) {
-        issue_recs(tile_of(j0), n & 1);
+        issue_recs(tile0, n & 1);
         issue_edges(hdr0.x, hdr_ne(hdr0), n & 1);
     }
-    if (j1 < nmy) { hdr1 = load_hdr(tile_of(j1)); hid1 = load_hid(tile_of(j1)); hint1 = ldcg_i32(act_prev + tile_of(j1)); }
-    gather_halo(tile_of(j0), hdr_nh(hdr0), hid0, n & 1);
+    if (tile1 >= 0) { hdr1 = load_hdr(tile1); hid1 = load_hid(tile1); hint1 = ldcg_i32(act_prev + tile1); }
+    gather_halo(tile0, hdr_nh(hdr0), hid0, n & 1);
     cp_async_commit();
-    for (;;) {
+    for (unsigned q = 0;; q++) {                          // q: stage of this step (n runs on across the steps of a launch)
         const int s = n & 1;
-        const int tile = tile_of(j0);
+        const int tile = tile0;
         const int base = tile * TC;
-        const bool have_next = j1 < nmy;
+        const bool have_next = tile1 >= 0;
         const int ne = hdr_ne(hdr0), nh = hdr_nh(hdr0);
         // ---- top
         cp_async_wait<0>();                               // own halo gathers of this tile
@@ -758,12 +844,12 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
         const int i = base + tid;
         bool wet = i < P.nt && srec[tid].h > hdry;
         if (tid < nh) wet |= srec[TC + tid].h > hdry;
-        for (int q = tid + TC; q < nh; q += TC) wet |= srec[TC + q].h > hdry;
+        for (int k = tid + TC; k < nh; k += TC) wet |= srec[TC + k].h > hdry;
         // barrier: everyone has left the previous tile; everyone's gathers are visible
         const bool active = __syncthreads_or(wet) || hdr0.w != 0;
         if (producer) {
             if (have_next) {
-                issue_recs(tile_of(j1), s ^ 1);
+                issue_recs(tile1, s ^ 1);
                 // Edge lists are 40 of the ~105 bytes a cell costs and an all-dry tile never reads its
                 // list, so the list of the NEXT tile is requested only if that tile was active at the
                 // previous step; a tile that turns out active without its list (the wet front reached
@@ -774,13 +860,8 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
             act_next[tile] = active;
             scount[0] += active; scount[3] += !active;
         }
-        if (have_next) gather_halo(tile_of(j1), hdr_nh(hdr1), hid1, s ^ 1);
+        if (have_next) gather_halo(tile1, hdr_nh(hdr1), hid1, s ^ 1);
         cp_async_commit();
-        // the stage after the next one: its header, halo id and hint into registers
-        const int j2 = have_next ? next_stage(j1 + 1) : nmy;
-        int4 hdr2 = make_int4(0, 0, 0, 0);
-        int hid2 = -1, hint2 = 0;
-        if (j2 < nmy) { hdr2 = load_hdr(tile_of(j2)); hid2 = load_hid(tile_of(j2)); hint2 = ldcg_i32(act_prev + tile_of(j2)); }
         // this tile's edge list: requested one tile ago, or fetched now if the tile is active without it
         if (!req0 && active && producer) issue_edges(hdr0.x, ne, s);
         if (req0 || active) {
@@ -792,6 +873,8 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
             // all fluxes vanish, h' = h + 0, and dry cells carry u = v = 0 already (R-15), so the
             // step leaves the records unchanged bit for bit.  The copy still moves them.
             if (i < P.nt) store_rec(Uout + i, srec[tid]);
+            if (producer) sring[(q + 2) & 3] = have_next ? claim_tile<QUIET>(P.wq, P.wlist, P.wstride, cs, sq, nmy) : -1;
+            __syncthreads();
         } else {
             // ---- phase 1: every edge of the tile once, shared memory only (a2-a7)
             const unsigned char *const se = sedge0 + s * estride;
@@ -817,7 +900,16 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
                     so2[sb] = -o[4];
                 }
             }
+            // the tile of the stage after the next one: claimed while the first warps finish their edges
+            if (producer) sring[(q + 2) & 3] = have_next ? claim_tile<QUIET>(P.wq, P.wlist, P.wstride, cs, sq, nmy) : -1;
             __syncthreads();
+        }
+        // the stage after the next one: its header, halo id and hint into registers
+        const int tile2 = sring[(q + 2) & 3];
+        int4 hdr2 = make_int4(0, 0, 0, 0);
+        int hid2 = -1, hint2 = 0;
+        if (tile2 >= 0) { hdr2 = load_hdr(tile2); hid2 = load_hid(tile2); hint2 = ldcg_i32(act_prev + tile2); }
+        if (active) {
             mbar_wait(bar + 4, cpar);                          // this tile's cell constants
             cpar ^= 1u;
             // ---- phase 2: every cell of the tile (a7-a10)
@@ -835,7 +927,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
         }
         if (!have_next) break;
         n++;
-        j0 = j1; j1 = j2;
+        tile0 = tile1; tile1 = tile2;
         hdr0 = hdr1; hid0 = hid1; req0 = hint1 != 0;
         hdr1 = hdr2; hid1 = hid2; hint1 = hint2;
     }

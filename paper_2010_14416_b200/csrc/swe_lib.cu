@@ -339,7 +339,7 @@ static_assert(sizeof(HostEdge) == 24 && kDevPosMask == kPosMask && kDevKShift ==
               kDevNoSlot == kNoSlot, "edge list encoding (mesh_builder.h / swe_kernels.cuh)");
 static_assert(kTileNbrs == kNbrs && sizeof(HostEdge) == sizeof(GEdge), "neighbour-tile rows / global edge records");
 struct Layout {
-    size_t U0, U1, cellc, edges, tinfo, bvol, act0, act1, tnbr, binact, zcell, perm, stage, pmax0, pmax1, qn, ctrl, gedges, cedge, eres, total;
+    size_t U0, U1, cellc, edges, tinfo, bvol, act0, act1, tnbr, binact, wq, wlist, zcell, perm, stage, pmax0, pmax1, qn, ctrl, gedges, cedge, eres, total;
 };
 Layout make_layout(const HostTables &T, const TileTables &X, const GlobalEdges &E)
 {
@@ -351,6 +351,7 @@ Layout make_layout(const HostTables &T, const TileTables &X, const GlobalEdges &
     L.bvol = take(((size_t)X.nbedges + 1) * sizeof(double));
     L.act0 = take(((size_t)X.ntiles + 1) * sizeof(int32_t)); L.act1 = take(((size_t)X.ntiles + 1) * sizeof(int32_t));
     L.tnbr = take(X.tnbr.size() * sizeof(int32_t)); L.binact = take(kMaxPart * sizeof(int32_t));
+    L.wq = take(kMaxPart * sizeof(unsigned long long)); L.wlist = take(((size_t)X.ntiles + kMaxPart) * sizeof(int32_t));
     L.zcell = take(n * sizeof(double)); L.perm = take(n * sizeof(int32_t));
     L.stage = take(3 * n * sizeof(double));
     L.pmax0 = take(kMaxPart * sizeof(double)); L.pmax1 = take(kMaxPart * sizeof(double));
@@ -500,9 +501,9 @@ int swe_get_step_bytes(const swe_mesh *m, double active_tiles, double edge_lists
         return SWE_OK;
     }
     double b = 0.0;
-    b += 32.0 * nt;                                   // every cell's record read (TMA bulk copy) ...
-    b += 32.0 * nt;                                   // ... and written (256-bit store)
     const double voting = std::max(0.0, ntiles - quiet_tiles);   // tiles that gather their halo and vote
+    b += 32.0 * nt * voting / ntiles;                 // their cells' records read (TMA bulk copy) ...
+    b += 32.0 * nt * voting / ntiles;                 // ... and written (256-bit store); quiet tiles are not touched
     b += 32.0 * (double)X.nhalo * voting / ntiles;    // halo records, one 32-byte sector each (mean list length)
     b += voting * (16.0 + 4.0 * (double)std::min(X.max_halo, X.tile_cells));   // header, halo ids
     b += ntiles * (4.0 + 4.0) + (ntiles - voting + active_tiles) * 4.0 * kNbrs;  // activity flag in and out, neighbour rows
@@ -629,6 +630,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.bvol = (double *)(m->ws + L.bvol);
     P.act0 = (int32_t *)(m->ws + L.act0); P.act1 = (int32_t *)(m->ws + L.act1);
     P.tnbr = (const int32_t *)(m->ws + L.tnbr); P.binact = (int32_t *)(m->ws + L.binact);
+    P.wq = (unsigned long long *)(m->ws + L.wq); P.wlist = (int32_t *)(m->ws + L.wlist);
     m->d_zcell = (double *)(m->ws + L.zcell); m->d_inv = (int32_t *)(m->ws + L.perm);
     m->d_stage = (double *)(m->ws + L.stage);
     P.pmax0 = (double *)(m->ws + L.pmax0); P.pmax1 = (double *)(m->ws + L.pmax1);
@@ -641,6 +643,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
     P.nge = (int32_t)m->E.edges.size();
     P.nt = (int32_t)T.nt; P.ntiles = ntiles; P.max_edges = X.max_edges; P.max_halo = X.max_halo;
     P.npart = mode == SWE_LOOP_PERSISTENT ? m->coop_grid : m->grid;
+    P.wstride = (ntiles + P.npart - 1) / std::max(P.npart, 1);
     P.g = m->prm.g; P.hg = 0.5 * m->prm.g; P.inv_g = 1.0 / m->prm.g; P.cfl = m->prm.cfl;
     // a side is dry iff h <= h_dry; the floor keeps every argument of the MUFU-seeded
     // reciprocal / rsqrt a normal number when the caller asks for h_dry = 0
@@ -664,6 +667,7 @@ int swe_mesh_bind_device(swe_mesh *m, void *device_workspace, size_t bytes, void
         CK(cudaMemsetAsync(P.pmax0, 0, kMaxPart * sizeof(double), s));
         CK(cudaMemsetAsync(P.pmax1, 0, kMaxPart * sizeof(double), s));
         CK(cudaMemsetAsync(P.ctrl, 0, sizeof(Ctrl), s));
+        CK(cudaMemsetAsync(P.wq, 0, kMaxPart * sizeof(unsigned long long), s));
         CK(cudaMemsetAsync(P.bvol, 0, ((size_t)X.nbedges + 1) * sizeof(double), s));
         CK(cudaStreamSynchronize(s));
     } catch (const std::bad_alloc &) { m->err = "out of host memory"; return SWE_ERR_NOMEM; }
