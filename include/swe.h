@@ -13,7 +13,7 @@
  * Conventions
  *   - Every function returns SWE_OK (0) or a negative swe_status; nothing throws across the
  *     ABI.  swe_last_error(mesh) gives a message for the last failure on that handle
- *     (swe_last_error(NULL): last failure of swe_mesh_create in this thread).
+ *     (swe_last_error(NULL): last failure of a call without a handle in this thread).
  *   - "host" pointers are ordinary CPU memory, caller-owned, read or written during the call
  *     only.  "device" pointers are CUDA device memory of the bound device, caller-owned.
  *   - Cells are addressed in the CALLER's numbering everywhere in this ABI; the internal
@@ -301,6 +301,27 @@ int swe_get_tile_tables(const swe_mesh *mesh, int32_t *edge_a, int32_t *edge_b, 
  * by this handle so far (step, rate, pack/unpack kernels). */
 int swe_get_launch_info(const swe_mesh *mesh, int32_t *grid, int32_t *block, int32_t *loop_mode,
                         int64_t *kernel_launches);
+
+/*
+ * The CFL time step of eq.(15) WITHOUT a handle, a workspace or any
+ * allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops,
+ * harnesses that forbid it): dt = cfl / max_i (sqrt(g h_i) + |(hu_i, hv_i)| / h_i) / inradius_i over
+ * the cells with h_i > h_dry, 0 if there is none.  The same quantity swe_compute_dt returns for that
+ * state (equal to rounding: the handle-based path stores velocities and 1/R).
+ *   d_h, d_hu, d_hv, d_inradius   device [n], any cell order (inradius as swe_get_tables returns it)
+ *   d_dt                          device, one double, written on the stream
+ *   cuda_stream                   cudaStream_t (NULL: the default stream); nothing is synchronised
+ * The per-block partial maxima live in a fixed device array inside the library (512 KiB per GPU that
+ * loads it, held until exit) sized for n <= SWE_STATIC_MAX_CELLS; a larger n is rejected with
+ * SWE_ERR_INVALID_ARG and a message in swe_last_error(NULL).  All calls share that array: calls that
+ * overlap on the GPU (different streams, no dependency between them) race on it; calls on one stream
+ * are safe, and a call does not depend on what the previous one left there.  Works on the device
+ * that is current at the call.  Calls no cudaMalloc / cudaFree / allocating routine.
+ * Errors: SWE_ERR_INVALID_ARG, SWE_ERR_CUDA (launch failure; message in swe_last_error(NULL)).
+ */
+#define SWE_STATIC_MAX_CELLS 67108864   /* 2^26 cells (the largest workload of the paper's kind here has 50M) */
+int swe_cfl_dt_static(const double *d_h, const double *d_hu, const double *d_hv, const double *d_inradius,
+                      int64_t n, double g, double cfl, double h_dry, double *d_dt, void *cuda_stream);
 
 const char *swe_last_error(const swe_mesh *mesh);
 

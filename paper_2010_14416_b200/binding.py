@@ -30,7 +30,7 @@ SYMBOLS = [
     "swe_compute_dt", "swe_step", "swe_run", "swe_run_until", "swe_get_boundary_volumes",
     "swe_snapshot_begin", "swe_snapshot_wait", "swe_sync", "swe_get_state", "swe_get_state_device",
     "swe_get_stats", "swe_get_permutation", "swe_get_tables", "swe_get_tile_info",
-    "swe_get_tile_tables", "swe_get_launch_info", "swe_get_step_bytes",
+    "swe_get_tile_tables", "swe_get_launch_info", "swe_get_step_bytes", "swe_cfl_dt_static",
     "swe_last_error",
 ]
 
@@ -95,6 +95,7 @@ def load_library(rebuild_if_stale: bool = True):
     L.swe_get_tile_tables.argtypes = [vp, i32p, i32p, dp, i32p]
     L.swe_get_launch_info.argtypes = [vp, i32p, i32p, i32p, C.POINTER(C.c_int64)]
     L.swe_get_step_bytes.argtypes = [vp, C.c_double, C.c_double, C.c_double, dp]
+    L.swe_cfl_dt_static.argtypes = [vp, vp, vp, vp, i64, C.c_double, C.c_double, C.c_double, vp, vp]
     L.swe_last_error.argtypes = [vp]
     L.swe_last_error.restype = C.c_char_p
     for name in SYMBOLS:
@@ -102,6 +103,15 @@ def load_library(rebuild_if_stale: bool = True):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
+
+
+def cfl_dt_static(d_h, d_hu, d_hv, d_inradius, n, g, cfl, h_dry, d_dt, stream=None):
+    """swe_cfl_dt_static (include/swe.h): the CFL time step with no handle and no allocation; all
+    arguments are device addresses (ints, e.g. tensor.data_ptr()); stream = cudaStream_t as int."""
+    L = load_library()
+    rc = L.swe_cfl_dt_static(d_h, d_hu, d_hv, d_inradius, n, g, cfl, h_dry, d_dt, stream)
+    if rc != 0:
+        raise SweError(rc, (L.swe_last_error(None) or b"").decode())
 
 
 def _dp(a):

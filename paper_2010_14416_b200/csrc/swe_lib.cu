@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1047,3 +1048,108 @@ int swe_get_stats(swe_mesh *m, swe_stats *s)
 }
 
 } // extern "C"
+
+// =================================================================================================
+// swe_cfl_dt_static: the CFL time step without any allocation (include/swe.h)
+// =================================================================================================
+// A variant of swe_rate_kernel + swe_finalize_dt_kernel for callers that cannot allocate (code under
+// CUDA graph capture, serving loops, harnesses that forbid cudaMalloc) and have no workspace to bind:
+// the per-block maxima, which the handle-based path keeps in the caller's workspace, live in a
+// file-scope device array of fixed size.  Every GPU that loads the library holds these 512 KiB until
+// exit.  In host code the array's NAME is a host-side stand-in, not a device address: the address a
+// kernel can use comes from cudaGetSymbolAddress, asked once per device with that device current.
+// Every call shares the array; it keeps the previous call's contents, which is harmless here because
+// a call writes each of the partials it later reads (nothing has to start at zero), but two calls
+// that overlap on the GPU (different streams) race on it.
+namespace {
+constexpr int kStaticThreads = 256, kStaticCellsPerThread = 4;
+constexpr int kStaticCellsPerBlock = kStaticThreads * kStaticCellsPerThread;              // 1024
+constexpr int64_t kStaticMaxCells = SWE_STATIC_MAX_CELLS;
+constexpr int kStaticMaxBlocks = (int)(kStaticMaxCells / kStaticCellsPerBlock);          // 65536 partial maxima
+static_assert(kStaticMaxCells % kStaticCellsPerBlock == 0, "SWE_STATIC_MAX_CELLS: a multiple of 1024");
+static __device__ __align__(256) double g_static_scratch[kStaticMaxBlocks];
+
+// pass 1: block b takes cells [1024 b, 1024 b + 1024); scratch[b] = its maximum of (sqrt(g h)+|V|)/R
+__global__ void __launch_bounds__(kStaticThreads)
+swe_static_rate_kernel(const double *__restrict__ h, const double *__restrict__ hu, const double *__restrict__ hv,
+                       const double *__restrict__ inradius, const long long n, const double g, const double hdry,
+                       double *__restrict__ scratch)
+{
+    __shared__ double s_red[32];
+    double rate = 0.0;
+    const long long base = (long long)blockIdx.x * kStaticCellsPerBlock + threadIdx.x;
+#pragma unroll
+    for (int q = 0; q < kStaticCellsPerThread; q++) {
+        const long long i = base + (long long)q * kStaticThreads;
+        if (i < n) {
+            const double hi = __ldg(h + i);
+            if (hi > hdry) {                                    // eq.(15) with d = R_i, wet cells only (R-15)
+                const double u = __ldg(hu + i) / hi, v = __ldg(hv + i) / hi;
+                rate = fmax(rate, (sqrt(g * hi) + sqrt(fma(u, u, v * v))) / __ldg(inradius + i));
+            }
+        }
+    }
+    rate = block_max(rate, s_red);
+    if (threadIdx.x == 0) scratch[blockIdx.x] = rate;
+}
+
+// pass 2: one block; dt = CFL / max of the nblk partials this call wrote (0 if every cell is dry)
+__global__ void __launch_bounds__(1024)
+swe_static_dt_kernel(const double *__restrict__ scratch, const int nblk, const double cfl, double *__restrict__ dt_out)
+{
+    __shared__ double s_red[32];
+    double r = 0.0;
+    for (int k = threadIdx.x; k < nblk; k += blockDim.x) r = fmax(r, scratch[k]);
+    r = block_max(r, s_red);
+    if (threadIdx.x == 0) *dt_out = r > 0.0 ? cfl / r : 0.0;
+}
+
+// device address of g_static_scratch on the current device, looked up once per device
+constexpr int kMaxDevices = 64;
+double *g_static_ptr[kMaxDevices] = {};
+std::mutex g_static_mutex;
+cudaError_t static_scratch_for_current_device(double **ptr)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        double *p = nullptr;
+        e = cudaGetSymbolAddress((void **)&p, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        g_static_ptr[dev] = p;
+    }
+    *ptr = g_static_ptr[dev];
+    return cudaSuccess;
+}
+} // namespace
+
+extern "C" int swe_cfl_dt_static(const double *d_h, const double *d_hu, const double *d_hv, const double *d_inradius,
+                                 int64_t n, double g, double cfl, double h_dry, double *d_dt, void *cuda_stream)
+{
+    if (!d_h || !d_hu || !d_hv || !d_inradius || !d_dt || n <= 0 || !(g > 0.0) || !(cfl > 0.0) || !(h_dry >= 0.0)) {
+        g_create_err = "swe_cfl_dt_static: NULL pointer, n <= 0 or a parameter out of range";
+        return SWE_ERR_INVALID_ARG;
+    }
+    if (n > kStaticMaxCells) {
+        g_create_err = "swe_cfl_dt_static: n = " + std::to_string(n) + " cells exceeds SWE_STATIC_MAX_CELLS = " +
+                       std::to_string(kStaticMaxCells) + " (the fixed scratch array holds one partial maximum per 1024 cells)";
+        return SWE_ERR_INVALID_ARG;
+    }
+    double *scratch = nullptr;
+    cudaError_t e = static_scratch_for_current_device(&scratch);
+    if (e == cudaSuccess) {
+        cudaStream_t s = (cudaStream_t)cuda_stream;
+        const int nblk = (int)((n + kStaticCellsPerBlock - 1) / kStaticCellsPerBlock);
+        swe_static_rate_kernel<<<nblk, kStaticThreads, 0, s>>>(d_h, d_hu, d_hv, d_inradius, (long long)n, g, h_dry, scratch);
+        swe_static_dt_kernel<<<1, 1024, 0, s>>>(scratch, nblk, cfl, d_dt);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) {
+        g_create_err = std::string("swe_cfl_dt_static: ") + cudaGetErrorString(e);
+        return SWE_ERR_CUDA;
+    }
+    return SWE_OK;
+}
