@@ -320,8 +320,11 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
     value = job_throughput(n, args.steps, world, ms)
     peak, peak_src = load_peaks()
     kernel_ms = ms / args.steps                       # one step kernel launch per step
-    sample, what = make_sample(args.workload)
-    cpu_value, cpu_threads, _ = time_oracle(sample, 10 if sample.ncells > 300000 else 100, 2)
+    if args.cpu_baseline:
+        sample, what = make_sample(args.workload)
+        cpu_value, cpu_threads, _ = time_oracle(sample, 10 if sample.ncells > 300000 else 100, 2)
+    else:                                   # profiling / sweep runs: the oracle leg is skipped and says so
+        cpu_value, cpu_threads, what = None, 0, "skipped (--no-cpu-baseline)"
 
     def l2_policy(cells):
         return "inputs larger than L2 (no flush)" if cells * 164 > 2 * 126e6 \
@@ -380,6 +383,8 @@ def main():
     ap.add_argument("--kernel", default="tiled", choices=["tiled", "edge"],
                     help="tiled = the fused tile kernel (default); edge = the edge-centric two-pass alternative (A/B only)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false",
+                    help="skip the oracle-on-host-cores leg (sweeps and runs under ncu; the default line carries it)")
     ap.add_argument("--no-wet", dest="wet", action="store_false",
                     help="skip the all-wet leg (config3) that the default run times beside the headline workload")
     args = ap.parse_args()
