@@ -117,6 +117,8 @@ typedef struct {
     int64_t quiet_tile_steps;  /* sum over the steps of the number of QUIET tiles: inactive in the previous step with
                                   all their neighbour tiles, hence all dry now, and with their records already in
                                   place in both state buffers: they are not touched */
+    int64_t stolen_tile_steps; /* sum over the steps of the number of tiles computed by a thread block other than the
+                                  one they are dealt to (work stealing); results do not depend on it */
 } swe_stats;
 
 /* Fills *p with the defaults listed above. */

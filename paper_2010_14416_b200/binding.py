@@ -45,7 +45,7 @@ class SweStats(C.Structure):
     _fields_ = [("volume", C.c_double), ("t", C.c_double), ("dt_last", C.c_double),
                 ("steps", C.c_int64), ("n_dry", C.c_int64), ("n_clamped", C.c_int64),
                 ("n_nonfinite", C.c_int64), ("active_tile_steps", C.c_int64),
-                ("edge_list_fetches", C.c_int64), ("quiet_tile_steps", C.c_int64)]
+                ("edge_list_fetches", C.c_int64), ("quiet_tile_steps", C.c_int64), ("stolen_tile_steps", C.c_int64)]
 
 
 class SweError(RuntimeError):

@@ -79,6 +79,7 @@ struct Ctrl {                 // device-resident loop state
     unsigned long long n_active;  // tiles that were not all dry, summed over the steps (diagnostics)
     unsigned long long n_elists;  // edge lists fetched, summed over the steps (diagnostics)
     unsigned long long n_quiet;   // quiet tiles (left untouched), summed over the steps (diagnostics)
+    unsigned long long n_stolen;  // tiles computed by a block other than their owner, summed over the steps (diagnostics)
     int all_dry;              // set when a step found no wet cell
     int bad_cell;             // smallest caller id with a negative depth or a non-finite value (swe_set_state)
 };
@@ -513,7 +514,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait()
 //   double  scell[3][TC]           1/|Omega|, 1/R, g m^2
 //   uint64  bar[5]                 rec[2], edge[2], cell constants
 //   uint32  count[4]               the producer thread's counters
-//   int32   ring[4], claim[4]      tiles of the coming pipeline stages; the producer thread's claim state
+//   int32   ring[4], claim[8]      tiles of the coming pipeline stages; the producer thread's claim state
 //   uint32  sq[128]                quiet flags of the block's tiles
 //   Rec     srec[2][TC + MH]       state records of the tile's cells, then of its halo cells
 //   uint2 + double2  sedge[2][ME]  the tile's edge list (24 bytes per edge)
@@ -539,7 +540,7 @@ template <int TC> struct SmemLayout {
     static constexpr int scell = (so2 + 3 * PLC * 8 + 15) & ~15;
     static constexpr int bar = scell + 3 * TC * 8;
     static constexpr int ring = bar + kNumBars * 8 + 16;                 // after four diagnostic counters
-    static constexpr int sq = ring + 32;                                 // after the ring and the claim state
+    static constexpr int sq = ring + 48;                                 // after the ring and the claim state
     static constexpr int srec = (sq + kMaxSeq / 8 + 31) & ~31;
 };
 __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int ME)
@@ -548,7 +549,7 @@ __host__ __device__ __forceinline__ size_t tile_smem_bytes(int TC, int MH, int M
     size_t o = 3 * PLC * 16;
     o = (o + 3 * PLC * 8 + 15) & ~(size_t)15;
     o += 3 * (size_t)TC * 8;
-    o = (o + kNumBars * 8 + 16 + 32 + 4096 / 8 + 31) & ~(size_t)31;      // barriers, counters, ring + claim state, quiet flags (kMaxSeq bits)
+    o = (o + kNumBars * 8 + 16 + 48 + 4096 / 8 + 31) & ~(size_t)31;      // barriers, counters, ring + claim state, quiet flags (kMaxSeq bits)
     o += 2 * (size_t)(TC + MH) * sizeof(Rec);
     o += 2 * (size_t)ME * 24;
     return o;
@@ -632,6 +633,8 @@ struct ClaimState {
     int jc;        // own list: next position of the block's sequence to look at
     int pre;       // own claims already contained in the initial work word
     int fails;     // probe rounds that found no victim since the last good claim
+    int stolen;    // tiles taken from other blocks' lists in this step (diagnostics)
+    int pad[3];
 };
 constexpr unsigned long long kTailOne = 1ull << 32;
 constexpr unsigned kListBit = 0x80000000u;
@@ -666,7 +669,7 @@ __device__ __noinline__ int claim_tile(unsigned long long *const wq, const int32
             const unsigned long long old = atomicAdd(wq + v, 0ull - kTailOne);
             const int h = (int)((unsigned)old & ~kListBit), t = (int)(unsigned)(old >> 32);
             if (h < t) {
-                cs->fails = 0;
+                cs->fails = 0; cs->stolen++;
                 if (!((unsigned)old & kListBit)) return v + (t - 1) * G;
                 __threadfence();            // the list was published before the word
                 return ldcg_i32(wlist + (size_t)v * wstride + (t - 1));
@@ -808,7 +811,7 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
     if (producer) {
         const int pre = min(len, 2);
         P.wq[blockIdx.x] = ((unsigned long long)(unsigned)len << 32) | (QUIET ? kListBit : 0u) | (unsigned)pre;
-        cs->src = blockIdx.x; cs->jc = 0; cs->pre = pre; cs->fails = 0;
+        cs->src = blockIdx.x; cs->jc = 0; cs->pre = pre; cs->fails = 0; cs->stolen = 0;
     }
     // the first two stages (a block with a shorter list of its own takes from others right away)
     if (producer) {

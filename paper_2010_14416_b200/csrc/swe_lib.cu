@@ -71,6 +71,8 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
             if (cnt[1]) { atomicAdd(&P.ctrl->n_elists, (unsigned long long)cnt[1]); cnt[1] = 0; }
             if (cnt[2]) { atomicAdd(&P.ctrl->n_quiet, (unsigned long long)cnt[2]); cnt[2] = 0; }
             P.binact[blockIdx.x] = (int)cnt[3]; cnt[3] = 0;
+            const int nst = reinterpret_cast<const ClaimState *>(dyn_smem + SmemLayout<TC>::ring + 16)->stolen;
+            if (nst > 0 && (int)blockIdx.x < P.ntiles) atomicAdd(&P.ctrl->n_stolen, (unsigned long long)nst);
         }
         if (threadIdx.x == 0) {
             P.pmax(cur ^ 1)[blockIdx.x] = rate;
@@ -1044,6 +1046,7 @@ int swe_get_stats(swe_mesh *m, swe_stats *s)
     s->active_tile_steps = (int64_t)c.n_active;
     s->edge_list_fetches = (int64_t)c.n_elists;
     s->quiet_tile_steps = (int64_t)c.n_quiet;
+    s->stolen_tile_steps = (int64_t)c.n_stolen;
     return SWE_OK;
 }
 

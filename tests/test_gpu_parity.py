@@ -314,9 +314,9 @@ def test_edge_two_pass_kernel_matches_oracle_and_tiled_kernel(loop_mode):
 
 def test_quiet_tiles_bitwise_against_the_kernels_without_shortcuts():
     """A mesh large enough for the quiet-tile path (blocks with >= 8 tiles, most of them on the dry
-    floodplain): the tile kernel copies all-dry tiles and streams quiet tiles through registers
-    without a halo gather, the edge-centric kernels compute every edge and every cell of every
-    step.  Identical bits, while the wet front keeps moving into quiet territory; and parity with
+    floodplain): the tile kernel copies all-dry tiles and leaves quiet tiles untouched (both state
+    buffers hold their records already), the edge-centric kernels compute every edge and every
+    cell of every step.  Identical bits, while the wet front keeps moving into quiet territory; and parity with
     the oracle at the usual bar."""
     w = W.config4(nx=1600, ny=400)
     m, o = run_both(w, 300, block_size=64)
@@ -340,6 +340,50 @@ def test_quiet_tiles_bitwise_against_the_kernels_without_shortcuts():
     for a, b in zip(got[:3], p.get_state()[:3]):
         np.testing.assert_array_equal(a, b)
     assert p.get_stats()["quiet_tile_steps"] == st["quiet_tile_steps"]
+
+
+def test_untouched_quiet_tiles_and_work_stealing_across_run_calls_and_a_new_state():
+    """Quiet tiles are not written, which is right only while both state buffers hold their records;
+    blocks take tiles from each other's lists, which must not change a bit.  Uneven swe_run calls
+    (the buffer parity flips between calls), read-backs in between, then a NEW state whose wet region
+    lies where the old one was quiet (swe_set_state must forget what the tiles were), against the
+    edge-centric kernels, which have neither shortcut, with the same sequence of calls."""
+    w = W.config4(nx=1600, ny=400)
+    t = B.SweMesh.from_workload(w, block_size=64).bind_device()
+    e = B.SweMesh.from_workload(w, kernel=B.KERNEL_EDGE_TWO_PASS).bind_device()
+
+    def both(fn):
+        return fn(t), fn(e)
+
+    def same_state():
+        a, b = both(lambda m: m.get_state())
+        for x, y in zip(a[:3], b[:3]):
+            np.testing.assert_array_equal(x, y)
+        assert a[3] == b[3] and a[4] == b[4]
+        return a
+
+    both(lambda m: m.set_state(w.h, w.hu, w.hv))
+    for chunk in (1, 2, 3, 7, 30, 1, 101):
+        both(lambda m: m.run(chunk))
+        same_state()
+    st, ti = t.get_stats(), t.get_tile_info()
+    assert st["steps"] == 145
+    assert st["quiet_tile_steps"] > 0.5 * 145 * ti["ntiles"]
+    assert st["stolen_tile_steps"] > 0                      # the wet channel is a small part of the mesh: idle blocks took tiles
+    assert e.get_stats()["stolen_tile_steps"] == 0
+    # a new state: the old one mirrored in y (the channel meanders, so water now stands on cells that were quiet)
+    h, hu, hv = same_state()[:3]
+    cy = W.centroids(w.nodes_xy, w.tris)[:, 1]
+    order = np.argsort(cy, kind="stable")
+    h2, hu2, hv2 = h.copy(), np.zeros_like(hu), np.zeros_like(hv)
+    h2[order] = h[order[::-1]]
+    assert np.count_nonzero((h2 > w.h_dry) & (h <= w.h_dry)) > 1000
+    both(lambda m: m.set_state(h2, hu2, hv2))
+    for chunk in (5, 64):
+        both(lambda m: m.run(chunk))
+        same_state()
+    assert t.get_stats()["n_clamped"] == e.get_stats()["n_clamped"]
+    np.testing.assert_array_equal(t.get_boundary_volumes(), e.get_boundary_volumes())
 
 
 def test_edge_two_pass_kernel_ordering_invariance_and_run_until():

@@ -26,7 +26,7 @@ def test_library_exports_every_declared_symbol():
 
 def test_struct_sizes_match_header():
     assert ctypes.sizeof(B.SweParams) == 3 * 8 + 6 * 4
-    assert ctypes.sizeof(B.SweStats) == 3 * 8 + 7 * 8
+    assert ctypes.sizeof(B.SweStats) == 3 * 8 + 8 * 8
     p = B.SweParams()
     B.load_library().swe_params_default(ctypes.byref(p))
     assert (p.g, p.cfl, p.h_dry, p.ordering, p.loop_mode) == (9.81, 0.9, 1e-6, B.ORDER_HILBERT, B.LOOP_AUTO)
