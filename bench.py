@@ -186,7 +186,7 @@ STATE_BYTES_DRY = 64.0        # an all-dry tile's update is the identity: its 32
 
 
 def roofline_record(n, kernel_ms, active_share, list_share, step_bytes, tiles, peak, peak_src, quiet_share=None,
-                    kernel_name=None):
+                    kernel_name=None, stolen_share=None):
     """HBM roofline of one launch of the step kernel (= one time step of the whole mesh).
 
     frac cannot exceed ~1 for a correct kernel: it charges the SURVEY's 156 algorithmic bytes only
@@ -208,6 +208,7 @@ def roofline_record(n, kernel_ms, active_share, list_share, step_bytes, tiles, p
             "algorithmic_bytes_per_launch": algo, "algorithmic_bytes_per_cell_active_tile": ALGO_BYTES_PER_CELL,
             "algorithmic_bytes_per_cell_dry_tile": STATE_BYTES_DRY, "algorithmic_bytes_per_cell_quiet_tile": 0.0,
             "active_tile_share": active_share, "edge_list_share": list_share, "quiet_tile_share": quiet_share,
+            "stolen_tile_share": stolen_share,
             "achieved_fixed_156": fixed / sec / 1e9, "frac_fixed_156": fixed / sec / 1e9 / peak,
             "frac_of_nominal_8TBs": algo / sec / 1e9 / 8000.0,
             "kernel": kernel_name or f"swe_step_kernel<{tiles['tile_cells']}>", "peak_source": peak_src}
@@ -250,9 +251,10 @@ def measure_device(B, w, args, dev, order, loop, barrier, world, sampler=None):
     active_share = (st["active_tile_steps"] - st0["active_tile_steps"]) / tile_steps
     list_share = (st["edge_list_fetches"] - st0["edge_list_fetches"]) / tile_steps
     quiet_share = (st["quiet_tile_steps"] - st0["quiet_tile_steps"]) / tile_steps
+    stolen_share = (st["stolen_tile_steps"] - st0["stolen_tile_steps"]) / tile_steps
     step_bytes = m.get_step_bytes(active_share * tiles["ntiles"], list_share * tiles["ntiles"],
                                   quiet_share * tiles["ntiles"])
-    return dict(quiet_share=quiet_share, mesh=m, ms=ms, clocks=clocks, info=info, tiles=tiles, launches=launches, stats=st,
+    return dict(quiet_share=quiet_share, stolen_share=stolen_share, mesh=m, ms=ms, clocks=clocks, info=info, tiles=tiles, launches=launches, stats=st,
                 active_share=active_share, list_share=list_share, step_bytes=step_bytes, t_build=t_build)
 
 
@@ -344,7 +346,8 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                    "n_clamped": stats["n_clamped"]},
         "roofline": roofline_record(n, kernel_ms, r["active_share"], r["list_share"], r["step_bytes"],
                                     tiles, peak, peak_src, r["quiet_share"],
-                                    "swe_edge_pass_kernel + swe_cell_pass_kernel" if args.kernel == "edge" else None),
+                                    "swe_edge_pass_kernel + swe_cell_pass_kernel" if args.kernel == "edge" else None,
+                                    r["stolen_share"]),
         "cpu_baseline": {"value": cpu_value, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
                          "sample": what, "value_1_thread": getattr(time_oracle, "one_thread", None),
                          "host_cores": os.cpu_count()},
@@ -364,7 +367,8 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
             "wet_fraction_end": 1.0 - r3["stats"]["n_dry"] / w3.ncells, "l2_policy": l2_policy(w3.ncells),
             "grid": r3["info"]["grid"], "block": r3["info"]["block"], "gpu_launches": r3["launches"],
             "roofline": roofline_record(w3.ncells, ms3 / args.steps, r3["active_share"], r3["list_share"],
-                                        r3["step_bytes"], r3["tiles"], peak, peak_src, r3["quiet_share"]),
+                                        r3["step_bytes"], r3["tiles"], peak, peak_src, r3["quiet_share"],
+                                        None, r3["stolen_share"]),
         }
     print(json.dumps(line), flush=True)
     if world > 1:
