@@ -628,6 +628,8 @@ __device__ __forceinline__ int next_nonquiet(const unsigned *sq, int j, const in
 // boundary accumulators), so they are the same bits with or without stealing.
 // All of it is done by the block's producer thread while its warp waits for the longer edge loops of
 // the first warps; the tile of the stage after the next one goes to the others through a ring.
+// Lists are shared only on meshes with at least kStealMinTiles tiles per block: below that a step is
+// one or two passes through the pipeline per block and probing from the prologue would only add latency.
 struct ClaimState {
     int src;       // list being consumed: own block first, then victims; -1: nothing left anywhere
     int jc;        // own list: next position of the block's sequence to look at
@@ -642,6 +644,10 @@ constexpr unsigned kListBit = 0x80000000u;
 #define SWE_PROBE_ROUNDS 2
 #endif
 constexpr int kProbe = 8, kProbeRounds = SWE_PROBE_ROUNDS;
+#ifndef SWE_STEAL_MIN_TILES
+#define SWE_STEAL_MIN_TILES 8
+#endif
+constexpr int kStealMinTiles = SWE_STEAL_MIN_TILES;   // tiles per block (mesh / grid) from which lists are shared
 
 template <bool QUIET>
 __device__ __noinline__ int claim_tile(unsigned long long *const wq, const int32_t *const wlist, const int wstride,
@@ -809,9 +815,13 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
         __syncthreads();
     }
     if (producer) {
-        const int pre = min(len, 2);
-        P.wq[blockIdx.x] = ((unsigned long long)(unsigned)len << 32) | (QUIET ? kListBit : 0u) | (unsigned)pre;
-        cs->src = blockIdx.x; cs->jc = 0; cs->pre = pre; cs->fails = 0; cs->stolen = 0;
+        // Meshes with only a few tiles per block are bound by the latency of one pass through the pipeline,
+        // and probing others' lists from the prologue would add to it: there the lists stay private (the
+        // whole list is pre-claimed, nobody probes; the criterion is the same for every block of the grid).
+        const bool steal = P.wstride >= kStealMinTiles;
+        const int pre = steal ? min(len, 2) : len;
+        if (steal) P.wq[blockIdx.x] = ((unsigned long long)(unsigned)len << 32) | (QUIET ? kListBit : 0u) | (unsigned)pre;
+        cs->src = blockIdx.x; cs->jc = 0; cs->pre = pre; cs->fails = steal ? 0 : kProbeRounds; cs->stolen = 0;
     }
     // the first two stages (a block with a shorter list of its own takes from others right away)
     if (producer) {
