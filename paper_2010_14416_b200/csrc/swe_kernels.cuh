@@ -897,8 +897,9 @@ __device__ __forceinline__ double step_tiles(const Params &P, unsigned char *sme
                 const uint2 ab = sab[e];
                 const double2 l = slxy[e];
                 const Rec A = srec[ab.x & kPosMask];
-                Rec B = A;
-                if ((int32_t)ab.y >= 0) B = srec[ab.y & kPosMask];
+                // (a boundary edge reads A again: B is not used there, and selecting the index costs one
+                // instruction where copying the record costs eight)
+                const Rec B = srec[((int32_t)ab.y >= 0 ? ab.y : ab.x) & kPosMask];
                 double o[5];
                 edge_eval(P, l.x, l.y, A, B, (int32_t)ab.y, dt, o);
                 // b's slot gets the negated values (its outward normal is -n)
@@ -1056,8 +1057,7 @@ __device__ __forceinline__ void cluster_loop(const Params &P, unsigned char *sme
                 const uint2 ab = sab[e];
                 const double2 l = slxy[e];
                 const Rec A = srec[ab.x & kPosMask];
-                Rec B = A;
-                if ((int32_t)ab.y >= 0) B = srec[ab.y & kPosMask];
+                const Rec B = srec[((int32_t)ab.y >= 0 ? ab.y : ab.x) & kPosMask];
                 double o[5];
                 edge_eval(P, l.x, l.y, A, B, (int32_t)ab.y, dt, o);
                 const unsigned sa = ab.x >> kSlotShift;
