@@ -209,6 +209,8 @@ def roofline_record(n, kernel_ms, active_share, list_share, step_bytes, tiles, p
             "algorithmic_bytes_per_cell_dry_tile": STATE_BYTES_DRY, "algorithmic_bytes_per_cell_quiet_tile": 0.0,
             "active_tile_share": active_share, "edge_list_share": list_share, "quiet_tile_share": quiet_share,
             "stolen_tile_share": stolen_share,
+            # cells of tiles that did the method's arithmetic, per second (value counts every cell of the mesh)
+            "active_cell_updates_per_s": active_share * n / sec,
             "achieved_fixed_156": fixed / sec / 1e9, "frac_fixed_156": fixed / sec / 1e9 / peak,
             "frac_of_nominal_8TBs": algo / sec / 1e9 / 8000.0,
             "kernel": kernel_name or f"swe_step_kernel<{tiles['tile_cells']}>", "peak_source": peak_src}
