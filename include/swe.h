@@ -246,6 +246,18 @@ int swe_get_state_device(swe_mesh *mesh, double *d_h, double *d_hu, double *d_hv
 int swe_snapshot_begin(swe_mesh *mesh, double *h, double *hu, double *hv, double *t);
 int swe_snapshot_wait(swe_mesh *mesh);
 
+/*
+ * Gauges: (h, hu, hv) of n cells, given by their caller ids, at the current time -- a water-level or discharge
+ * record at fixed points costs 28 bytes per gauge instead of a read-back of the whole state (the paper streams
+ * its per-step diagnostics to the host beside the computation).  The values are the ones
+ * swe_get_state returns for those cells, bit for bit.
+ *   cells host [n], 0 <= id < nt, 1 <= n <= max(1, nt / 2);  h, hu, hv host [n];  t may be NULL
+ * Synchronises the stream; waits for a pending snapshot (the samples pass through the same staging buffer).
+ * Errors: SWE_ERR_INVALID_ARG, SWE_ERR_BAD_INDEX (id out of range), SWE_ERR_NOT_BOUND, SWE_ERR_NO_STATE.
+ */
+int swe_sample_cells(swe_mesh *mesh, const int32_t *cells, int64_t n, double *h, double *hu, double *hv,
+                     double *t);
+
 /* Diagnostics (synchronises, copies h to the host). */
 int swe_get_stats(swe_mesh *mesh, swe_stats *stats);
 

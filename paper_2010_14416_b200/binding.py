@@ -30,7 +30,7 @@ SYMBOLS = [
     "swe_compute_dt", "swe_step", "swe_run", "swe_run_until", "swe_get_boundary_volumes",
     "swe_snapshot_begin", "swe_snapshot_wait", "swe_sync", "swe_get_state", "swe_get_state_device",
     "swe_get_stats", "swe_get_permutation", "swe_get_tables", "swe_get_tile_info",
-    "swe_get_tile_tables", "swe_get_launch_info", "swe_get_step_bytes", "swe_cfl_dt_static",
+    "swe_get_tile_tables", "swe_get_launch_info", "swe_get_step_bytes", "swe_cfl_dt_static", "swe_sample_cells",
     "swe_last_error",
 ]
 
@@ -88,6 +88,7 @@ def load_library(rebuild_if_stale: bool = True):
     L.swe_get_state.argtypes = [vp, dp, dp, dp, dp, dp]
     L.swe_get_state_device.argtypes = [vp, vp, vp, vp]
     L.swe_get_stats.argtypes = [vp, C.POINTER(SweStats)]
+    L.swe_sample_cells.argtypes = [vp, i32p, i64, dp, dp, dp, dp]
     L.swe_get_permutation.argtypes = [vp, i32p]
     L.swe_get_tables.argtypes = [vp, i32p, dp, dp, dp, dp, dp]
     L.swe_get_tile_info.argtypes = [vp, i32p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), i32p, i32p,
@@ -284,6 +285,16 @@ class SweMesh:
         self._ck(self._L.swe_get_state_device(self._h, C.c_void_p(d_h.data_ptr()),
                                               C.c_void_p(d_hu.data_ptr()),
                                               C.c_void_p(d_hv.data_ptr())))
+
+    def sample_cells(self, cells):
+        """Gauges: (h, hu, hv, t) of the given cells (caller ids) at the current time."""
+        cells = np.ascontiguousarray(cells, dtype=np.int32)
+        n = cells.size
+        h, hu, hv = np.empty(n), np.empty(n), np.empty(n)
+        t = C.c_double(0)
+        self._ck(self._L.swe_sample_cells(self._h, cells.ctypes.data_as(C.POINTER(C.c_int32)), n, _dp(h), _dp(hu), _dp(hv),
+                                          C.byref(t)))
+        return h, hu, hv, t.value
 
     def get_stats(self) -> dict:
         s = SweStats()

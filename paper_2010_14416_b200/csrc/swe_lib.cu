@@ -291,6 +291,16 @@ __global__ void swe_unpack_kernel(const Params P, const int cur, const int32_t *
     if (hu) hu[c] = r.h * r.u;
     if (hv) hv[c] = r.h * r.v;
 }
+// swe_sample_cells: (h, hu, hv) of n cells given by caller ids (gauges); out = [3][n]
+template <class R>
+__global__ void swe_sample_kernel(const Params P, const int cur, const int32_t *__restrict__ inv,
+                                  const int32_t *__restrict__ cells, const int n, double *__restrict__ out)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const Rec r = ldrec<R>(reinterpret_cast<const R *>(P.U(cur)) + inv[cells[k]]);
+    out[k] = r.h; out[n + k] = r.h * r.u; out[2 * n + k] = r.h * r.v;
+}
 
 } // namespace
 
@@ -1018,6 +1028,36 @@ int swe_get_state(swe_mesh *m, double *h, double *hu, double *hv, double *t, dou
     if (rc != SWE_OK) return rc;
     if (t) *t = c.t[m->cur];
     if (dt_next) *dt_next = c.dt;
+    return SWE_OK;
+}
+
+int swe_sample_cells(swe_mesh *m, const int32_t *cells, int64_t n, double *h, double *hu, double *hv, double *t)
+{
+    if (!m || !cells || !h || !hu || !hv || n <= 0) return SWE_ERR_INVALID_ARG;
+    if (!m->bound) { m->err = "no device workspace bound"; return SWE_ERR_NOT_BOUND; }
+    if (!m->have_state) { m->err = "no state set"; return SWE_ERR_NO_STATE; }
+    const int64_t nt = m->T.nt;
+    if (n > std::max<int64_t>(1, nt / 2)) { m->err = "swe_sample_cells: at most half the cells (swe_get_state reads them all)"; return SWE_ERR_INVALID_ARG; }
+    for (int64_t k = 0; k < n; k++)
+        if (cells[k] < 0 || cells[k] >= nt) { m->err = "swe_sample_cells: cell id out of range at position " + std::to_string(k); return SWE_ERR_BAD_INDEX; }
+    int rc = snapshot_finish(m);       // the samples pass through the staging buffer
+    if (rc != SWE_OK) return rc;
+    // staging buffer: [3][n] doubles out, the ids behind the first two thirds of it
+    double *d_out = m->d_stage;
+    int32_t *d_cells = reinterpret_cast<int32_t *>(m->d_stage + 2 * (size_t)nt);
+    CK(cudaMemcpyAsync(d_cells, cells, (size_t)n * sizeof(int32_t), cudaMemcpyHostToDevice, m->stream));
+    const unsigned nb = (unsigned)((n + 127) / 128);
+    if (m->f32) swe_sample_kernel<RecF><<<nb, 128, 0, m->stream>>>(m->P, m->cur, m->d_inv, d_cells, (int)n, d_out);
+    else swe_sample_kernel<Rec><<<nb, 128, 0, m->stream>>>(m->P, m->cur, m->d_inv, d_cells, (int)n, d_out);
+    m->launches++;
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(h, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+    CK(cudaMemcpyAsync(hu, d_out + n, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+    CK(cudaMemcpyAsync(hv, d_out + 2 * n, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, m->stream));
+    Ctrl c;
+    rc = read_ctrl(m, &c, false);      // synchronises the stream
+    if (rc != SWE_OK) return rc;
+    if (t) *t = c.t[m->cur];
     return SWE_OK;
 }
 

@@ -669,6 +669,46 @@ def test_locally_refined_mesh():
         o2.run(37)
 
 
+def test_gauges_sample_cells_against_get_state_and_oracle():
+    """swe_sample_cells: a gauge record (h, hu, hv at fixed cells) taken at three stages of the wet-dry dam break
+    equals swe_get_state at those cells bit for bit and the oracle's state at the usual bar; ids are checked."""
+    w = W.config2(nx=300, ny=30)
+    m = B.SweMesh.from_workload(w).bind_device()
+    o = OracleSolver.from_workload(w)
+    m.set_state(w.h, w.hu, w.hv)
+    rng = np.random.default_rng(5)
+    cells = np.concatenate([[0, w.ncells - 1], rng.choice(w.ncells, 200, replace=False)]).astype(np.int32)
+    for stage in range(3):
+        m.run(120)
+        assert o.run(120) == 120
+        gh, ghu, ghv, gt = m.sample_cells(cells)
+        h, hu, hv, t, _ = m.get_state()
+        np.testing.assert_array_equal(gh, h[cells])
+        np.testing.assert_array_equal(ghu, hu[cells])
+        np.testing.assert_array_equal(ghv, hv[cells])
+        assert gt == t
+        ho, huo, hvo, to, _ = o.get_state()
+        np.testing.assert_allclose(gh, ho[cells], rtol=RTOL, atol=ATOL)
+        np.testing.assert_allclose(ghu, huo[cells], rtol=RTOL, atol=ATOL)
+        np.testing.assert_allclose(ghv, hvo[cells], rtol=RTOL, atol=ATOL)
+        assert gt == pytest.approx(to, rel=1e-12)
+    assert np.count_nonzero(gh > w.h_dry) > 20 and np.count_nonzero(gh <= w.h_dry) > 20     # gauges on both sides of the front
+    for bad in ([-1], [w.ncells], []):
+        with pytest.raises(B.SweError):
+            m.sample_cells(bad)
+    with pytest.raises(B.SweError):
+        m.sample_cells(np.arange(w.ncells // 2 + 1))
+    # single-precision storage on the edge-centric kernels: the same read path
+    e = B.SweMesh.from_workload(w, kernel=B.KERNEL_EDGE_TWO_PASS, fp_kind=B.FP_MIXED32).bind_device()
+    e.set_state(w.h, w.hu, w.hv)
+    e.run(50)
+    gh, ghu, ghv, _ = e.sample_cells(cells)
+    h, hu, hv = e.get_state()[:3]
+    np.testing.assert_array_equal(gh, h[cells])
+    np.testing.assert_array_equal(ghu, hu[cells])
+    np.testing.assert_array_equal(ghv, hv[cells])
+
+
 def test_active_tile_counter():
     """swe_stats.active_tile_steps: every tile of an all-wet mesh is active at every step; on the
     wet-dry dam break the dry end of the canal is not, and the count grows as the front advances."""
