@@ -50,11 +50,12 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
     __syncthreads();
     PipeState it;
     for (long long s = 0; s < nsteps; s++) {
-        const int ninact = ldcg_i32(P.binact + blockIdx.x);      // (in flight during the reduction below)
+        // (these loads are in flight during the reduction below)
+        const int ninact = ldcg_i32(P.binact + blockIdx.x);
+        const double t_now = __ldcg(&P.ctrl->t[cur]), t_end = __ldcg(&P.ctrl->t_end);
         const double dt_cfl = reduce_dt(P, P.pmax(cur), s_red);
         // swe_run_until: the step that would pass t_end ends on it; after that, zero steps
-        const double t_now = __ldcg(&P.ctrl->t[cur]);
-        const double left = __ldcg(&P.ctrl->t_end) - t_now;
+        const double left = t_end - t_now;
         const bool clipped = dt_cfl >= left;
         const double dt = fmax(clipped ? left : dt_cfl, 0.0);
         unsigned nclamp = 0;
@@ -79,7 +80,7 @@ swe_step_kernel(const Params P, int cur, const long long nsteps)
             if (blockIdx.x == 0) {
                 Ctrl *c = P.ctrl;
                 // R-24: the clipped step ends ON t_end (t + (t_end - t) may round off it)
-                c->t[cur ^ 1] = clipped ? fmax(__ldcg(&P.ctrl->t_end), t_now) : t_now + dt;
+                c->t[cur ^ 1] = clipped ? fmax(t_end, t_now) : t_now + dt;
                 if (dt > 0.0) { c->dt_last = dt; c->steps += 1; }
                 if (!(dt_cfl > 0.0)) c->all_dry = 1;
             }
