@@ -386,6 +386,29 @@ def test_untouched_quiet_tiles_and_work_stealing_across_run_calls_and_a_new_stat
     np.testing.assert_array_equal(t.get_boundary_volumes(), e.get_boundary_volumes())
 
 
+def test_full_size_river_graph_and_persistent_loops_bitwise_whatever_is_stolen():
+    """BASELINE configs[3] at full size (13 M cells, bench.py's launch configuration): the CUDA-graph loop and the
+    cooperative persistent loop give the same bits and skip the same quiet tiles, although which block computes
+    which tile depends on timing (the stolen-tile counts of two runs differ)."""
+    w = W.config4()
+    res = []
+    for loop_mode in (B.LOOP_GRAPH, B.LOOP_PERSISTENT):
+        m = B.SweMesh.from_workload(w, loop_mode=loop_mode).bind_device()
+        m.set_state(w.h, w.hu, w.hv)
+        for chunk in (1, 7, 192):
+            m.run(chunk)
+        res.append((m.get_state(), m.get_stats()))
+        m.destroy()
+    (a, sa), (b, sb) = res
+    for x, y in zip(a[:3], b[:3]):
+        np.testing.assert_array_equal(x, y)
+    assert a[3] == b[3] and a[4] == b[4]
+    assert sa["steps"] == sb["steps"] == 200
+    assert sa["quiet_tile_steps"] == sb["quiet_tile_steps"] > 0
+    assert sa["active_tile_steps"] == sb["active_tile_steps"] > 0
+    assert sa["stolen_tile_steps"] > 0 and sb["stolen_tile_steps"] > 0
+
+
 def test_edge_two_pass_kernel_ordering_invariance_and_run_until():
     w = W.config2(nx=300, ny=30)
     out = []
