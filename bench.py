@@ -345,7 +345,11 @@ def run_gpu(args, rank: int, world: int, local_rank: int):
                    "smem_bytes_per_block": tiles["smem_bytes"], "l2_policy": l2_policy(n),
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "mesh_build_s": round(r["t_build"], 2), "wet_fraction_end": 1.0 - stats["n_dry"] / n,
-                   "n_clamped": stats["n_clamped"]},
+                   "n_clamped": stats["n_clamped"],
+                   "counts": "every cell of the mesh per step; all-dry tiles whose neighbourhood was dry a step ago "
+                             "(roofline.quiet_tile_share) are left untouched because their update is the identity and "
+                             "both state buffers hold it: the state after K steps is bit for bit what computing every "
+                             "cell gives (tests/test_gpu_parity.py); 'wet' is the regime without any shortcut"},
         "roofline": roofline_record(n, kernel_ms, r["active_share"], r["list_share"], r["step_bytes"],
                                     tiles, peak, peak_src, r["quiet_share"],
                                     "swe_edge_pass_kernel + swe_cell_pass_kernel" if args.kernel == "edge" else None,
