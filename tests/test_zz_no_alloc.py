@@ -65,6 +65,28 @@ def test_static_scratch_dt_matches_compute_dt_twice_in_a_row():
 
 
 @pytest.mark.gpu
+def test_static_scratch_dt_against_the_oracle():
+    """The oracle's own eq.(15) on its own geometry (inradius included), for a state with velocities."""
+    import torch
+    from oracle.swe_oracle import OracleSolver
+    w = W.canal_dam_break(120, 12, h_left=1.0, h_right=0.3, seed=9)          # 2880 cells
+    o = OracleSolver.from_workload(w)
+    o.run(25)                                   # get some velocities
+    h, hu, hv = o.get_state()[:3]
+    o2 = OracleSolver.from_workload(w)
+    o2.set_state(h, hu, hv)
+    dt_ref = o2.compute_dt()
+    rin = o.geometry()["rin"]
+    dev = torch.device("cuda", 0)
+    t = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (h, hu, hv, rin)]
+    out = torch.zeros(1, dtype=torch.float64, device=dev)
+    B.cfl_dt_static(t[0].data_ptr(), t[1].data_ptr(), t[2].data_ptr(), t[3].data_ptr(), w.ncells, w.g, w.cfl, w.h_dry,
+                    out.data_ptr(), None)
+    torch.cuda.synchronize()
+    assert dt_ref > 0.0 and float(out.item()) == pytest.approx(dt_ref, rel=1e-12)
+
+
+@pytest.mark.gpu
 def test_static_scratch_all_dry_gives_zero():
     import torch
     dev = torch.device("cuda", 0)
